@@ -1,0 +1,135 @@
+/* prefixflow.h -- C ABI of the B200-native attention hot path of PrefixFlow's training-time KV
+ * cache (arxiv/paper_2606_01143).  Citations are PAPER.md:<line> of the paper text.
+ *
+ * A GRPO rollout group is N trajectories [P || S(1)] ... [P || S(N)] that share one prefix P of
+ * Lp tokens.  The three-phase schedule runs, per attention
+ * layer:
+ *   Phase A  one causal forward over P; its K1/V1 become the training-time KV cache  (:152)
+ *   Phase B  for every suffix S(i): attention forward and backward whose queries read the cached
+ *            K1/V1 plus their own causal K2/V2 (:154-158, eq. :192); the gradients that reach the
+ *            prefix,  gV1 = P21^T dO2,  gK1 = sigma dS21^T Q2  (eq. :196), are ACCUMULATED over
+ *            the N suffixes (:162, :212)
+ *   Phase C  one delayed causal backward over P whose dK1/dV1 = own-prefix term + accumulated
+ *            gK1/gV1 (:160, :222)
+ * Only K1,V1 (read) and gK1,gV1 (written) cross the prefix/suffix boundary (Property 1, :190-200).
+ *
+ * Conventions:
+ *   - all pointers are DEVICE pointers unless a parameter name ends in _host; the library never
+ *     allocates or frees user tensors; every call only enqueues work on `stream`
+ *     (a cudaStream_t passed as void*), never synchronises, never allocates device memory;
+ *   - activations are bf16, token-major [L, H, d] with d contiguous and explicit token / head
+ *     strides in ELEMENTS (pf_tensor); base pointers and strides must be multiples of 8 elements
+ *     (16 bytes, a TMA requirement) -> PF_INVALID_ARG otherwise;
+ *   - LSE is fp32 [Hq, L] row-major (row stride = L), natural log of the sum of exp of the SCALED
+ *     scores; GQA head mapping kappa(h) = h / (Hq/Hkv); causal = key j <= query t (inclusive);
+ *   - gK1 / gV1 are fp32, contiguous [Lp, Hkv, d], borrowed for the lifetime of the group;
+ *   - head_dim in {64, 128}; softmax_scale 0 means 1/sqrt(head_dim);
+ *   - functions return a pf_status; nothing throws or aborts across this boundary; validation
+ *     happens before any launch; Ls = 0 and Lp = 0 are legal.
+ */
+#ifndef PREFIXFLOW_H_
+#define PREFIXFLOW_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pf_ctx pf_ctx;     /* opaque: device properties, driver entry points, options */
+typedef struct pf_group pf_group; /* opaque: one rollout group's training-time KV cache (:164) */
+typedef int32_t pf_status;
+
+enum {
+    PF_OK = 0,
+    PF_INVALID_ARG = 1, /* NULL / negative size / misaligned pointer or stride / Hq % Hkv != 0 */
+    PF_UNSUPPORTED = 2, /* head_dim not in {64,128}, non-contiguous accumulator, ... */
+    PF_CUDA_ERROR = 3,  /* a CUDA runtime / driver call failed; see pf_last_error */
+    PF_WORKSPACE = 4,   /* workspace NULL, misaligned or smaller than pf_workspace_bytes */
+    PF_STATE = 5        /* phase order violated (B or C before A, anything after C / end) */
+};
+
+typedef struct {
+    int32_t n_q_heads;   /* Hq */
+    int32_t n_kv_heads;  /* Hkv, divides Hq */
+    int32_t head_dim;    /* d: 64 or 128 */
+    float softmax_scale; /* sigma; 0 -> 1/sqrt(d) */
+} pf_desc;
+
+typedef struct {
+    void* ptr;           /* device pointer, element [0,0,0] */
+    int64_t stride_tok;  /* elements between consecutive tokens */
+    int64_t stride_head; /* elements between consecutive heads */
+} pf_tensor;
+
+int32_t pf_version(void);
+
+/* Create / destroy a context bound to CUDA device `device` (host-side state only). */
+pf_status pf_create(pf_ctx** out, int32_t device);
+pf_status pf_destroy(pf_ctx* ctx);
+/* Message of the last failing call on this context (valid until the next call). */
+const char* pf_last_error(const pf_ctx* ctx);
+/* Options (host-side, take effect at the next launch):
+ *   "bwd_head_parts" : split the G query heads of a KV head over this many CTAs per key tile in
+ *                      the backward (0 = heuristic).  1 = every key tile owned by one CTA
+ *                      (gK1/gV1 += without contention), G = maximal parallelism, most atomics. */
+pf_status pf_set_option(pf_ctx* ctx, const char* name, int64_t value);
+
+/* Bytes of caller-provided scratch needed by a group with prefix length Lp whose longest Phase-B
+ * call carries max_Ls suffix tokens (fp32 dQ / dK2 / dV2 staging and softmax statistics). */
+size_t pf_workspace_bytes(const pf_desc* desc, int64_t Lp, int64_t max_Ls);
+
+/* Open a group: register the cache K1,V1 [Lp,Hkv,d] bf16 (borrowed, immutable until
+ * pf_group_end) and the accumulators gK1,gV1 [Lp,Hkv,d] fp32 contiguous (borrowed; zeroed here,
+ * asynchronously on `stream`).  gK1.ptr and gV1.ptr may both be NULL: then
+ * Phase B is not allowed and Phase C runs without injection (the N-times replay baseline).
+ * `workspace` must be 256-byte aligned device memory of >= pf_workspace_bytes(desc, Lp, max_Ls)
+ * for every later call of this group; it may be shared by groups that never overlap in time. */
+pf_status pf_group_begin(pf_ctx* ctx, const pf_desc* desc, int64_t Lp, pf_tensor K1, pf_tensor V1,
+                         pf_tensor gK1, pf_tensor gV1, void* workspace, size_t workspace_bytes,
+                         void* stream, pf_group** out);
+
+/* Phase A: O1[t,h] = softmax_{j<=t}(sigma q1[h,t].k1[g,j]) v1[g,j], LSE1 [Hq,Lp].
+ * Q1, O1: [Lp,Hq,d] bf16. */
+pf_status pf_phaseA_fwd(pf_group* grp, pf_tensor Q1, pf_tensor O1, float* LSE1, void* stream);
+
+/* Phase B forward: for each of the n_seqs suffixes packed back to back along
+ * the token axis (cu_seqlens_host[n_seqs+1], cu[0] = 0; the usual case is n_seqs = 1), the
+ * queries of suffix i attend to all Lp cached prefix keys and causally to the keys of suffix i
+ * only.  Q2,O2: [sumLs,Hq,d]; K2,V2: [sumLs,Hkv,d]; LSE2: [Hq,sumLs].  K1/V1 are read in place
+ * (no concatenation copy).  cu_seqlens_dev is reserved (may be NULL). */
+pf_status pf_phaseB_fwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens_dev,
+                        const int32_t* cu_seqlens_host, pf_tensor Q2, pf_tensor K2, pf_tensor V2,
+                        pf_tensor O2, float* LSE2, void* stream);
+
+/* Phase B backward: dQ2 [sumLs,Hq,d], dK2, dV2 [sumLs,Hkv,d] bf16 of the
+ * suffix tokens, and   gK1 += sigma dS21^T Q2,  gV1 += P21^T dO2   (summed over the G query heads
+ * of each KV head; fp32; the accumulators persist across calls).  Calls of one
+ * group must be stream-ordered or on streams the caller orders. */
+pf_status pf_phaseB_bwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens_dev,
+                        const int32_t* cu_seqlens_host, pf_tensor Q2, pf_tensor K2, pf_tensor V2,
+                        pf_tensor O2, const float* LSE2, pf_tensor dO2, pf_tensor dQ2,
+                        pf_tensor dK2, pf_tensor dV2, void* stream);
+
+/* Phase C: causal backward over the prefix; dQ1 [Lp,Hq,d] and
+ * dK1 = bf16(own-prefix term + gK1), dV1 = bf16(own-prefix term + gV1), the sum taken in fp32
+ * and rounded once.  Side effect: on return gK1/gV1 hold that fp32 sum. */
+pf_status pf_phaseC_bwd(pf_group* grp, pf_tensor Q1, pf_tensor O1, const float* LSE1,
+                        pf_tensor dO1, pf_tensor dQ1, pf_tensor dK1, pf_tensor dV1, void* stream);
+
+/* Close the group (host-side; frees the handle only; enqueued work keeps running). */
+pf_status pf_group_end(pf_group* grp);
+
+/* Optional memory lifecycle: move a dormant prefix tensor (contiguous bytes)
+ * to / from PINNED host memory on a side stream while Phase B runs.  Plain async copies; the
+ * caller orders them against compute with events. */
+pf_status pf_offload(pf_ctx* ctx, const void* src_dev, void* dst_pinned_host, size_t bytes,
+                     void* side_stream);
+pf_status pf_prefetch(pf_ctx* ctx, const void* src_pinned_host, void* dst_dev, size_t bytes,
+                      void* side_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PREFIXFLOW_H_ */

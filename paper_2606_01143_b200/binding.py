@@ -1,0 +1,229 @@
+"""Thin ctypes binding of the C-ABI library (include/prefixflow.h), same names as the C calls.
+
+Argument marshalling only: every step of the path runs in the CUDA kernels behind the ABI.
+PyTorch tensors are used as device-memory handles (data_ptr + strides) and torch streams as
+cudaStream_t handles.  There is NO fallback: if libprefixflow.so is missing or a call fails, a
+PrefixFlowError is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+SO_PATH = os.path.join(_HERE, "libprefixflow.so")
+
+PF_OK, PF_INVALID_ARG, PF_UNSUPPORTED, PF_CUDA_ERROR, PF_WORKSPACE, PF_STATE = range(6)
+STATUS_NAMES = {0: "PF_OK", 1: "PF_INVALID_ARG", 2: "PF_UNSUPPORTED", 3: "PF_CUDA_ERROR",
+                4: "PF_WORKSPACE", 5: "PF_STATE"}
+
+# every symbol include/prefixflow.h declares
+SYMBOLS = ("pf_version", "pf_create", "pf_destroy", "pf_last_error", "pf_set_option",
+           "pf_workspace_bytes", "pf_group_begin", "pf_phaseA_fwd", "pf_phaseB_fwd",
+           "pf_phaseB_bwd", "pf_phaseC_bwd", "pf_group_end", "pf_offload", "pf_prefetch")
+
+
+class PrefixFlowError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"{STATUS_NAMES.get(status, status)}: {msg}")
+        self.status = status
+
+
+class pf_desc(ctypes.Structure):
+    _fields_ = [("n_q_heads", ctypes.c_int32), ("n_kv_heads", ctypes.c_int32),
+                ("head_dim", ctypes.c_int32), ("softmax_scale", ctypes.c_float)]
+
+
+class pf_tensor(ctypes.Structure):
+    _fields_ = [("ptr", ctypes.c_void_p), ("stride_tok", ctypes.c_int64),
+                ("stride_head", ctypes.c_int64)]
+
+
+_lib = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libprefixflow.so (built by `python -m paper_2606_01143_b200.build`)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(SO_PATH):
+        raise PrefixFlowError(PF_CUDA_ERROR, f"{SO_PATH} not built; run "
+                              "`python -m paper_2606_01143_b200.build` (no fallback path exists)")
+    L = ctypes.CDLL(SO_PATH)
+    vp, i32, i64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64
+    T = pf_tensor
+    pi32 = ctypes.POINTER(ctypes.c_int32)
+    L.pf_version.restype = i32
+    L.pf_version.argtypes = []
+    L.pf_create.restype = i32
+    L.pf_create.argtypes = [ctypes.POINTER(vp), i32]
+    L.pf_destroy.restype = i32
+    L.pf_destroy.argtypes = [vp]
+    L.pf_last_error.restype = ctypes.c_char_p
+    L.pf_last_error.argtypes = [vp]
+    L.pf_set_option.restype = i32
+    L.pf_set_option.argtypes = [vp, ctypes.c_char_p, i64]
+    L.pf_workspace_bytes.restype = ctypes.c_size_t
+    L.pf_workspace_bytes.argtypes = [ctypes.POINTER(pf_desc), i64, i64]
+    L.pf_group_begin.restype = i32
+    L.pf_group_begin.argtypes = [vp, ctypes.POINTER(pf_desc), i64, T, T, T, T, vp, ctypes.c_size_t,
+                                 vp, ctypes.POINTER(vp)]
+    L.pf_phaseA_fwd.restype = i32
+    L.pf_phaseA_fwd.argtypes = [vp, T, T, vp, vp]
+    L.pf_phaseB_fwd.restype = i32
+    L.pf_phaseB_fwd.argtypes = [vp, i32, pi32, pi32, T, T, T, T, vp, vp]
+    L.pf_phaseB_bwd.restype = i32
+    L.pf_phaseB_bwd.argtypes = [vp, i32, pi32, pi32, T, T, T, T, vp, T, T, T, T, vp]
+    L.pf_phaseC_bwd.restype = i32
+    L.pf_phaseC_bwd.argtypes = [vp, T, T, vp, T, T, T, T, vp]
+    L.pf_group_end.restype = i32
+    L.pf_group_end.argtypes = [vp]
+    L.pf_offload.restype = i32
+    L.pf_offload.argtypes = [vp, vp, vp, ctypes.c_size_t, vp]
+    L.pf_prefetch.restype = i32
+    L.pf_prefetch.argtypes = [vp, vp, vp, ctypes.c_size_t, vp]
+    _lib = L
+    return L
+
+
+# ---------------------------------------------------------------------------------------------
+# marshalling helpers
+# ---------------------------------------------------------------------------------------------
+
+def as_tensor(t: Optional[torch.Tensor], dtype=torch.bfloat16) -> pf_tensor:
+    """[L, H, d] torch tensor -> pf_tensor (pointer + element strides); None -> NULL."""
+    if t is None:
+        return pf_tensor(None, 0, 0)
+    if t.dim() != 3 or t.dtype != dtype:
+        raise PrefixFlowError(PF_INVALID_ARG, f"expected a 3-D {dtype} tensor, got {tuple(t.shape)} {t.dtype}")
+    if t.shape[2] > 1 and t.stride(2) != 1:
+        raise PrefixFlowError(PF_INVALID_ARG, "last dimension must be contiguous")
+    return pf_tensor(t.data_ptr() if t.numel() > 0 else None, t.stride(0), t.stride(1))
+
+
+def _ptr(t: Optional[torch.Tensor]):
+    return None if t is None or t.numel() == 0 else t.data_ptr()
+
+
+def _stream(stream) -> Optional[int]:
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    if isinstance(stream, torch.cuda.Stream):
+        return stream.cuda_stream or None
+    return int(stream) or None
+
+
+def _cu(cu_seqlens_host: Sequence[int]):
+    arr = (ctypes.c_int32 * len(cu_seqlens_host))(*[int(x) for x in cu_seqlens_host])
+    return arr
+
+
+def make_desc(n_q_heads: int, n_kv_heads: int, head_dim: int, softmax_scale: float = 0.0) -> pf_desc:
+    return pf_desc(int(n_q_heads), int(n_kv_heads), int(head_dim), float(softmax_scale))
+
+
+class _Handle:
+    """Opaque pf_ctx* / pf_group* plus the owning context (for pf_last_error)."""
+
+    def __init__(self, ptr: int, ctx: Optional["_Handle"] = None):
+        self.ptr = ptr
+        self.ctx = ctx
+
+
+def _check(status: int, ctx: Optional[_Handle]):
+    if status != PF_OK:
+        msg = lib().pf_last_error(ctx.ptr if ctx else None)
+        raise PrefixFlowError(status, msg.decode() if msg else "")
+
+
+# ---------------------------------------------------------------------------------------------
+# the C calls, one Python function each
+# ---------------------------------------------------------------------------------------------
+
+def pf_version() -> int:
+    return int(lib().pf_version())
+
+
+def pf_create(device: int = 0) -> _Handle:
+    out = ctypes.c_void_p()
+    st = lib().pf_create(ctypes.byref(out), int(device))
+    if st != PF_OK:
+        raise PrefixFlowError(st, f"pf_create(device={device}) failed (needs an sm_100 GPU)")
+    return _Handle(out.value)
+
+
+def pf_destroy(ctx: _Handle) -> None:
+    _check(lib().pf_destroy(ctx.ptr), None)
+    ctx.ptr = None
+
+
+def pf_last_error(ctx: _Handle) -> str:
+    return lib().pf_last_error(ctx.ptr).decode()
+
+
+def pf_set_option(ctx: _Handle, name: str, value: int) -> None:
+    _check(lib().pf_set_option(ctx.ptr, name.encode(), int(value)), ctx)
+
+
+def pf_workspace_bytes(desc: pf_desc, Lp: int, max_Ls: int) -> int:
+    return int(lib().pf_workspace_bytes(ctypes.byref(desc), int(Lp), int(max_Ls)))
+
+
+def pf_group_begin(ctx: _Handle, desc: pf_desc, Lp: int, K1, V1, gK1, gV1, workspace: torch.Tensor,
+                   stream=None) -> _Handle:
+    out = ctypes.c_void_p()
+    st = lib().pf_group_begin(ctx.ptr, ctypes.byref(desc), int(Lp), as_tensor(K1), as_tensor(V1),
+                              as_tensor(gK1, torch.float32), as_tensor(gV1, torch.float32),
+                              _ptr(workspace), workspace.numel() * workspace.element_size(),
+                              _stream(stream), ctypes.byref(out))
+    _check(st, ctx)
+    return _Handle(out.value, ctx)
+
+
+def pf_phaseA_fwd(grp: _Handle, Q1, O1, LSE1, stream=None) -> None:
+    _check(lib().pf_phaseA_fwd(grp.ptr, as_tensor(Q1), as_tensor(O1), _ptr(LSE1), _stream(stream)),
+           grp.ctx)
+
+
+def pf_phaseB_fwd(grp: _Handle, cu_seqlens_host: Sequence[int], Q2, K2, V2, O2, LSE2,
+                  stream=None, cu_seqlens_dev: Optional[torch.Tensor] = None) -> None:
+    cu = _cu(cu_seqlens_host)
+    _check(lib().pf_phaseB_fwd(grp.ptr, len(cu_seqlens_host) - 1,
+                               ctypes.cast(_ptr(cu_seqlens_dev), ctypes.POINTER(ctypes.c_int32)), cu,
+                               as_tensor(Q2), as_tensor(K2), as_tensor(V2), as_tensor(O2),
+                               _ptr(LSE2), _stream(stream)), grp.ctx)
+
+
+def pf_phaseB_bwd(grp: _Handle, cu_seqlens_host: Sequence[int], Q2, K2, V2, O2, LSE2, dO2, dQ2, dK2,
+                  dV2, stream=None, cu_seqlens_dev: Optional[torch.Tensor] = None) -> None:
+    cu = _cu(cu_seqlens_host)
+    _check(lib().pf_phaseB_bwd(grp.ptr, len(cu_seqlens_host) - 1,
+                               ctypes.cast(_ptr(cu_seqlens_dev), ctypes.POINTER(ctypes.c_int32)), cu,
+                               as_tensor(Q2), as_tensor(K2), as_tensor(V2), as_tensor(O2),
+                               _ptr(LSE2), as_tensor(dO2), as_tensor(dQ2), as_tensor(dK2),
+                               as_tensor(dV2), _stream(stream)), grp.ctx)
+
+
+def pf_phaseC_bwd(grp: _Handle, Q1, O1, LSE1, dO1, dQ1, dK1, dV1, stream=None) -> None:
+    _check(lib().pf_phaseC_bwd(grp.ptr, as_tensor(Q1), as_tensor(O1), _ptr(LSE1), as_tensor(dO1),
+                               as_tensor(dQ1), as_tensor(dK1), as_tensor(dV1), _stream(stream)),
+           grp.ctx)
+
+
+def pf_group_end(grp: _Handle) -> None:
+    _check(lib().pf_group_end(grp.ptr), grp.ctx)
+    grp.ptr = None
+
+
+def pf_offload(ctx: _Handle, src_dev: torch.Tensor, dst_pinned_host: torch.Tensor, stream) -> None:
+    nbytes = src_dev.numel() * src_dev.element_size()
+    _check(lib().pf_offload(ctx.ptr, _ptr(src_dev), _ptr(dst_pinned_host), nbytes, _stream(stream)), ctx)
+
+
+def pf_prefetch(ctx: _Handle, src_pinned_host: torch.Tensor, dst_dev: torch.Tensor, stream) -> None:
+    nbytes = dst_dev.numel() * dst_dev.element_size()
+    _check(lib().pf_prefetch(ctx.ptr, _ptr(src_pinned_host), _ptr(dst_dev), nbytes, _stream(stream)), ctx)

@@ -1,0 +1,307 @@
+// attn_fwd.cuh -- sm_100a attention forward with two KV sources.
+//
+//   O[t,h] = softmax_j( sigma <q[h,t], k[g,j]> ) v[g,j],   LSE[h,t] = log sum_j exp(sigma <q,k>)
+//
+// KV source 1 ("prefix", length Lp): every key is visible to every query (cached K1/V1, read in
+// place -- no concat copy).  KV source 2 ("causal", same length as the queries): key j visible to
+// query t iff j <= t.  Phase A / replay: Lp = 0.  Phase B: source 1 = cached prefix.
+//
+// One CTA = two query tiles of 128 rows ("slots": consecutive (row block, q head) items of one KV
+// head, so both read the same K/V stream) ping-ponged on the tensor core:
+//   warps 0-3  softmax of slot 0   (thread r <-> query row r <-> TMEM lane r)
+//   warps 4-7  softmax of slot 1
+//   warp  8    TMA producer (Q once, K/V tiles through a 2-stage ring)
+//   warp  9    tcgen05.mma issuer (one thread)
+// TMEM (512 columns): S0 | S1 | O0 | O1, 128 fp32 columns each; P (bf16) overwrites the first 64
+// columns of its S and is consumed from TMEM as the A operand of P.V.
+#pragma once
+#include <cuda.h>
+#include "sm100_ptx.cuh"
+
+namespace pf {
+
+struct FwdParams {
+    __nv_bfloat16* O;
+    int64_t o_stride_tok, o_stride_head;  // elements
+    float* LSE;                           // [Hq, lse_stride]
+    int64_t lse_stride;
+    int Lq;        // queries (= causal-source keys)
+    int Lp;        // prefix-source keys (0: none)
+    int Hq, Hkv, G;
+    int nRB;       // ceil(Lq / 128)
+    float scale_log2;  // sigma * log2(e)
+};
+
+template <int D>
+struct FwdCfg {
+    static constexpr int KS = 2;                       // K/V ring depth
+    static constexpr int TILE = 128 * D * 2;           // bytes of one 128 x D bf16 tile
+    static constexpr int SUB = 128 * 64 * 2;           // one 128 x 64 swizzle-128B sub-tile
+    static constexpr int NSUB = D / 64;
+    static constexpr int OFF_Q = 0;                    // 2 tiles
+    static constexpr int OFF_K = 2 * TILE;             // KS tiles
+    static constexpr int OFF_V = OFF_K + KS * TILE;    // KS tiles
+    static constexpr int OFF_BAR = OFF_V + KS * TILE;
+    static constexpr int SMEM = OFF_BAR + 256;
+    static constexpr int THREADS = 320;
+};
+
+template <int D>
+__global__ void __launch_bounds__(320, 1)
+attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK1,
+                const __grid_constant__ CUtensorMap tmV1, const __grid_constant__ CUtensorMap tmK2,
+                const __grid_constant__ CUtensorMap tmV2, const FwdParams p) {
+    using C = FwdCfg<D>;
+    extern __shared__ __align__(1024) uint8_t smem[];
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::OFF_BAR);
+    uint64_t* bar_Q = bars;                 // [2]
+    uint64_t* bar_Kf = bars + 2;            // [KS]
+    uint64_t* bar_Ke = bars + 4;
+    uint64_t* bar_Vf = bars + 6;
+    uint64_t* bar_Ve = bars + 8;
+    uint64_t* bar_S = bars + 10;            // [2] S_s ready (MMA -> softmax)
+    uint64_t* bar_P = bars + 12;            // [2] P_s ready (softmax -> MMA)
+    uint64_t* bar_done = bars + 14;         // all MMAs complete
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 16);
+
+    const int tid = threadIdx.x, warp = tid >> 5;
+    if ((smem_u32(smem) & 1023u) != 0) __trap();
+
+    // ---- work decode: items of KV head g are (rb, h') with index rb*G + h'; heaviest first ----
+    const int g = blockIdx.y;
+    const int nItems = p.nRB * p.G;
+    const int idx0 = nItems - 1 - 2 * int(blockIdx.x);
+    const int idx1 = idx0 - 1;                       // < 0: slot 1 idle
+    const int rb0 = idx0 / p.G, h0 = g * p.G + idx0 % p.G;
+    const int rb1 = idx1 >= 0 ? idx1 / p.G : -1, h1 = idx1 >= 0 ? g * p.G + idx1 % p.G : 0;
+    const int nP = (p.Lp + 127) >> 7;
+    const int n_iter0 = nP + rb0 + 1;                // slot 0 is the longer one
+    const int n_iter1 = idx1 >= 0 ? nP + rb1 + 1 : 0;
+
+    if (tid == 0) {
+        mbar_init(&bar_Q[0], 1); mbar_init(&bar_Q[1], 1);
+        for (int s = 0; s < C::KS; ++s) {
+            mbar_init(&bar_Kf[s], 1); mbar_init(&bar_Ke[s], 1);
+            mbar_init(&bar_Vf[s], 1); mbar_init(&bar_Ve[s], 1);
+        }
+        mbar_init(&bar_S[0], 1); mbar_init(&bar_S[1], 1);
+        mbar_init(&bar_P[0], 128); mbar_init(&bar_P[1], 128);
+        mbar_init(bar_done, 1);
+        fence_mbar_init();
+    }
+    if (warp == 8) {
+        tmem_alloc(tmem_slot, 512);
+        if (elect_one()) {
+            tma_prefetch_desc(&tmQ); tma_prefetch_desc(&tmK1); tma_prefetch_desc(&tmV1);
+            tma_prefetch_desc(&tmK2); tma_prefetch_desc(&tmV2);
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+
+    if (warp == 8) {
+        // =============================== TMA producer ===============================
+        if (elect_one()) {
+            mbar_arrive_expect_tx(&bar_Q[0], C::TILE);
+            for (int k = 0; k < C::NSUB; ++k)
+                tma_load_3d(smem + C::OFF_Q + k * C::SUB, &tmQ, &bar_Q[0], 64 * k, h0, rb0 * 128);
+            if (idx1 >= 0) {
+                mbar_arrive_expect_tx(&bar_Q[1], C::TILE);
+                for (int k = 0; k < C::NSUB; ++k)
+                    tma_load_3d(smem + C::OFF_Q + C::TILE + k * C::SUB, &tmQ, &bar_Q[1], 64 * k, h1,
+                                rb1 * 128);
+            }
+            for (int it = 0; it < n_iter0; ++it) {
+                const int st = it % C::KS;
+                const uint32_t ph = (it / C::KS) & 1;
+                const bool pre = it < nP;
+                const int row0 = (pre ? it : it - nP) * 128;
+                mbar_wait(&bar_Ke[st], ph ^ 1);
+                mbar_arrive_expect_tx(&bar_Kf[st], C::TILE);
+                for (int k = 0; k < C::NSUB; ++k)
+                    tma_load_3d(smem + C::OFF_K + st * C::TILE + k * C::SUB, pre ? &tmK1 : &tmK2,
+                                &bar_Kf[st], 64 * k, g, row0);
+                mbar_wait(&bar_Ve[st], ph ^ 1);
+                mbar_arrive_expect_tx(&bar_Vf[st], C::TILE);
+                for (int k = 0; k < C::NSUB; ++k)
+                    tma_load_3d(smem + C::OFF_V + st * C::TILE + k * C::SUB, pre ? &tmV1 : &tmV2,
+                                &bar_Vf[st], 64 * k, g, row0);
+            }
+        }
+    } else if (warp == 9) {
+        // =============================== MMA issuer ===============================
+        if (elect_one()) {
+            constexpr uint32_t idesc_qk = make_idesc_bf16(128, 128, false, false);
+            constexpr uint32_t idesc_pv = make_idesc_bf16(128, D, false, true);
+            const uint32_t sQ = smem_u32(smem + C::OFF_Q), sK = smem_u32(smem + C::OFF_K),
+                           sV = smem_u32(smem + C::OFF_V);
+            auto issue_S = [&](int s, int st) {  // S_s = Q_s . K^T
+                const uint32_t q = sQ + s * C::TILE, k = sK + st * C::TILE;
+#pragma unroll
+                for (int kk = 0; kk < D / 16; ++kk) {
+                    const uint32_t off = (kk >> 2) * C::SUB + (kk & 3) * 32;
+                    mma_ss(tmem + s * 128, make_smem_desc_sw128(q + off, 16, 1024),
+                           make_smem_desc_sw128(k + off, 16, 1024), idesc_qk, kk > 0);
+                }
+            };
+            auto issue_PV = [&](int s, int st, bool acc) {  // O_s += P_s . V
+                const uint32_t v = sV + st * C::TILE;
+#pragma unroll
+                for (int kk = 0; kk < 8; ++kk)
+                    mma_ts(tmem + 256 + s * D, tmem + s * 128 + kk * 8,
+                           make_smem_desc_sw128(v + kk * 2048, C::SUB, 1024), idesc_pv,
+                           (acc || kk > 0) ? 1u : 0u);
+            };
+            mbar_wait(&bar_Q[0], 0);
+            mbar_wait(&bar_Kf[0], 0);
+            tc_fence_after();
+            issue_S(0, 0);
+            mma_commit(&bar_S[0]);
+            if (n_iter1 > 0) {
+                mbar_wait(&bar_Q[1], 0);
+                tc_fence_after();
+                issue_S(1, 0);
+                mma_commit(&bar_S[1]);
+            }
+            mma_commit(&bar_Ke[0]);
+            for (int it = 0; it < n_iter0; ++it) {
+                const int st = it % C::KS;
+                const uint32_t ph = (it / C::KS) & 1;
+                const bool next = it + 1 < n_iter0;
+                const int st1 = (it + 1) % C::KS;
+                const uint32_t ph1 = ((it + 1) / C::KS) & 1;
+                mbar_wait(&bar_Vf[st], ph);
+                mbar_wait(&bar_P[0], it & 1);
+                tc_fence_after();
+                issue_PV(0, st, it > 0);
+                if (next) {
+                    mbar_wait(&bar_Kf[st1], ph1);
+                    tc_fence_after();
+                    issue_S(0, st1);
+                    mma_commit(&bar_S[0]);
+                }
+                if (it < n_iter1) {
+                    mbar_wait(&bar_P[1], it & 1);
+                    tc_fence_after();
+                    issue_PV(1, st, it > 0);
+                }
+                mma_commit(&bar_Ve[st]);
+                if (next) {
+                    if (it + 1 < n_iter1) {
+                        issue_S(1, st1);
+                        mma_commit(&bar_S[1]);
+                    }
+                    mma_commit(&bar_Ke[st1]);
+                }
+            }
+            mma_commit(bar_done);
+        }
+    } else {
+        // =============================== softmax warpgroups ===============================
+        const int s = warp >> 2;                 // slot
+        const int r = tid & 127;                 // row in tile == TMEM lane
+        const int n_iter = s == 0 ? n_iter0 : n_iter1;
+        const int rb = s == 0 ? rb0 : rb1;
+        const int h = s == 0 ? h0 : h1;
+        const int t = rb * 128 + r;              // global query row
+        const uint32_t lane_off = uint32_t((warp & 3) * 32) << 16;
+        const uint32_t tS = tmem + s * 128 + lane_off;
+        const uint32_t tO = tmem + 256 + s * D + lane_off;
+        float m_used = -INFINITY, l = 0.f;
+        for (int it = 0; it < n_iter; ++it) {
+            mbar_wait(&bar_S[s], it & 1);
+            tc_fence_after();
+            uint32_t x[4][32];
+            tmem_ld32(tS + 0, x[0]);
+            tmem_ld32(tS + 32, x[1]);
+            tmem_ld32(tS + 64, x[2]);
+            tmem_ld32(tS + 96, x[3]);
+            tmem_wait_ld();
+            int limit;
+            if (it < nP) limit = p.Lp - it * 128;
+            else limit = t - (it - nP) * 128 + 1;
+            if (limit < 128) {  // ragged prefix tail or causal diagonal
+#pragma unroll
+                for (int c = 0; c < 4; ++c)
+#pragma unroll
+                    for (int j = 0; j < 32; ++j)
+                        if (c * 32 + j >= limit) x[c][j] = 0xff800000u;  // -inf
+            }
+            float mx = -INFINITY;
+#pragma unroll
+            for (int c = 0; c < 4; ++c)
+#pragma unroll
+                for (int j = 0; j < 32; ++j) mx = fmaxf(mx, __uint_as_float(x[c][j]));
+            const float m_new = mx * p.scale_log2;
+            // lazy rescale: keep a stale max while the new one is within 2^8 of it
+            const bool need = (it == 0) || (m_new > m_used + 8.f);
+            if (__any_sync(0xffffffffu, need && it > 0)) {
+                const float alpha = need ? fast_exp2(m_used - m_new) : 1.f;
+                l *= alpha;
+#pragma unroll
+                for (int c = 0; c < D / 32; ++c) {
+                    uint32_t o[32];
+                    tmem_ld32(tO + c * 32, o);
+                    tmem_wait_ld();
+#pragma unroll
+                    for (int j = 0; j < 32; ++j) o[j] = __float_as_uint(__uint_as_float(o[j]) * alpha);
+                    tmem_st32(tO + c * 32, o);
+                }
+            }
+            if (need) m_used = m_new;
+            float sum = 0.f;
+#pragma unroll
+            for (int c = 0; c < 2; ++c) {
+                uint32_t pk[32];
+#pragma unroll
+                for (int j = 0; j < 32; ++j) {
+                    const int col = c * 64 + 2 * j;
+                    const float p0 = fast_exp2(fmaf(__uint_as_float(x[col >> 5][col & 31]),
+                                                    p.scale_log2, -m_used));
+                    const float p1 = fast_exp2(fmaf(__uint_as_float(x[(col + 1) >> 5][(col + 1) & 31]),
+                                                    p.scale_log2, -m_used));
+                    sum += p0 + p1;
+                    pk[j] = pack_bf16(p0, p1);
+                }
+                tmem_st32(tS + c * 32, pk);
+            }
+            l += sum;
+            tmem_wait_st();
+            tc_fence_before();
+            mbar_arrive(&bar_P[s]);
+        }
+        if (n_iter > 0) {
+            mbar_wait(bar_done, 0);
+            tc_fence_after();
+            const float inv = 1.f / l;
+            const bool valid = t < p.Lq;
+            __nv_bfloat16* orow = p.O + int64_t(t) * p.o_stride_tok + int64_t(h) * p.o_stride_head;
+#pragma unroll
+            for (int c = 0; c < D / 32; ++c) {
+                uint32_t o[32];
+                tmem_ld32(tO + c * 32, o);
+                tmem_wait_ld();
+                if (valid) {
+#pragma unroll
+                    for (int j = 0; j < 32; j += 8) {
+                        uint4 v;
+                        v.x = pack_bf16(__uint_as_float(o[j + 0]) * inv, __uint_as_float(o[j + 1]) * inv);
+                        v.y = pack_bf16(__uint_as_float(o[j + 2]) * inv, __uint_as_float(o[j + 3]) * inv);
+                        v.z = pack_bf16(__uint_as_float(o[j + 4]) * inv, __uint_as_float(o[j + 5]) * inv);
+                        v.w = pack_bf16(__uint_as_float(o[j + 6]) * inv, __uint_as_float(o[j + 7]) * inv);
+                        *reinterpret_cast<uint4*>(orow + c * 32 + j) = v;
+                    }
+                }
+            }
+            if (valid)
+                p.LSE[int64_t(h) * p.lse_stride + t] = (m_used + log2f(l)) * 0.6931471805599453f;
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 8) tmem_dealloc(tmem, 512);
+}
+
+}  // namespace pf

@@ -1,0 +1,595 @@
+// prefixflow.cu -- the C ABI declared in include/prefixflow.h: argument validation, TMA
+// descriptors, workspace carving and kernel launches.  No arithmetic of the method lives on the
+// host; every step runs in the kernels of attn_fwd.cuh / attn_bwd.cuh / aux_kernels.cuh.
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <cmath>
+#include <new>
+
+#include "../../include/prefixflow.h"
+#include "attn_fwd.cuh"
+#include "attn_bwd.cuh"
+#include "aux_kernels.cuh"
+
+namespace {
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*,
+                                  const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+constexpr int64_t kAlign = 256;
+inline int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
+
+}  // namespace
+
+struct pf_ctx {
+    int device = 0;
+    int num_sms = 0;
+    EncodeTiledFn encode = nullptr;
+    int bwd_head_parts = 0;  // 0 = heuristic
+    bool attr_set = false;
+    char err[512] = {0};
+};
+
+struct pf_group {
+    pf_ctx* ctx;
+    pf_desc desc;
+    float sigma;
+    int64_t Lp;
+    pf_tensor K1, V1;
+    float* gK1;
+    float* gV1;
+    uint8_t* ws;
+    size_t ws_bytes;
+    int state;  // 0 begun, 1 A done, 2 C done
+};
+
+namespace {
+
+pf_status fail(pf_ctx* ctx, pf_status st, const char* fmt, ...) {
+    if (ctx) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(ctx->err, sizeof(ctx->err), fmt, ap);
+        va_end(ap);
+    }
+    return st;
+}
+
+#define PF_CUDA(ctx, call)                                                              \
+    do {                                                                                \
+        cudaError_t e_ = (call);                                                        \
+        if (e_ != cudaSuccess)                                                          \
+            return fail(ctx, PF_CUDA_ERROR, "%s failed: %s", #call, cudaGetErrorString(e_)); \
+    } while (0)
+
+pf_status check_desc(pf_ctx* ctx, const pf_desc* d) {
+    if (!d) return fail(ctx, PF_INVALID_ARG, "desc is NULL");
+    if (d->n_q_heads <= 0 || d->n_kv_heads <= 0 || d->n_q_heads % d->n_kv_heads != 0)
+        return fail(ctx, PF_INVALID_ARG, "n_q_heads=%d must be a positive multiple of n_kv_heads=%d",
+                    d->n_q_heads, d->n_kv_heads);
+    if (d->head_dim != 64 && d->head_dim != 128)
+        return fail(ctx, PF_UNSUPPORTED, "head_dim=%d not in {64,128}", d->head_dim);
+    if (!(d->softmax_scale >= 0.f) || std::isinf(d->softmax_scale))
+        return fail(ctx, PF_INVALID_ARG, "softmax_scale must be finite and >= 0");
+    if (d->n_q_heads > 65535) return fail(ctx, PF_UNSUPPORTED, "n_q_heads > 65535");
+    return PF_OK;
+}
+
+// bf16 [L, H, d] strided tensor: pointer / stride rules of the TMA tiled mode
+pf_status check_tensor(pf_ctx* ctx, const char* name, const pf_tensor& t, int64_t L, int H, int d) {
+    if (L == 0) return PF_OK;
+    if (!t.ptr) return fail(ctx, PF_INVALID_ARG, "%s.ptr is NULL", name);
+    if (reinterpret_cast<uintptr_t>(t.ptr) % 16 != 0)
+        return fail(ctx, PF_INVALID_ARG, "%s.ptr must be 16-byte aligned", name);
+    if (t.stride_tok < d || t.stride_tok % 8 != 0)
+        return fail(ctx, PF_INVALID_ARG, "%s.stride_tok=%lld must be >= d and a multiple of 8", name,
+                    (long long)t.stride_tok);
+    if (H > 1 && (t.stride_head < d || t.stride_head % 8 != 0))
+        return fail(ctx, PF_INVALID_ARG, "%s.stride_head=%lld must be >= d and a multiple of 8", name,
+                    (long long)t.stride_head);
+    if (t.stride_tok * 2 >= (int64_t(1) << 40) || t.stride_head * 2 >= (int64_t(1) << 40))
+        return fail(ctx, PF_INVALID_ARG, "%s strides too large", name);
+    return PF_OK;
+}
+
+// 3-D map {d, H, L}, box {64, 1, 128}, swizzle-128B: one load = a [128 tokens][64 elements]
+// K-major sub-tile of one head; rows past L are zero-filled.
+pf_status make_map(pf_ctx* ctx, CUtensorMap* m, const char* name, const pf_tensor& t, int64_t L,
+                   int H, int d) {
+    if (L == 0) {
+        memset(m, 0, sizeof(*m));
+        return PF_OK;
+    }
+    cuuint64_t dims[3] = {cuuint64_t(d), cuuint64_t(H), cuuint64_t(L)};
+    cuuint64_t strides[2] = {cuuint64_t((H > 1 ? t.stride_head : int64_t(d)) * 2),
+                             cuuint64_t(t.stride_tok * 2)};
+    cuuint32_t box[3] = {64, 1, 128};
+    cuuint32_t es[3] = {1, 1, 1};
+    CUresult r = ctx->encode(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, t.ptr, dims, strides, box, es,
+                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                             CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS)
+        return fail(ctx, PF_CUDA_ERROR, "cuTensorMapEncodeTiled(%s) failed with CUresult %d", name,
+                    int(r));
+    return PF_OK;
+}
+
+struct WsLayout {
+    int64_t off_lse2, off_delta, off_dq, off_ak, off_av, total;
+    int64_t stat_stride;
+};
+
+WsLayout ws_layout(const pf_desc& d, int64_t Lmax) {
+    WsLayout w;
+    w.stat_stride = align_up(Lmax, 128);
+    int64_t o = 0;
+    w.off_lse2 = o; o += align_up(int64_t(d.n_q_heads) * w.stat_stride * 4, kAlign);
+    w.off_delta = o; o += align_up(int64_t(d.n_q_heads) * w.stat_stride * 4, kAlign);
+    w.off_dq = o; o += align_up(Lmax * d.n_q_heads * d.head_dim * 4, kAlign);
+    w.off_ak = o; o += align_up(Lmax * d.n_kv_heads * d.head_dim * 4, kAlign);
+    w.off_av = o; o += align_up(Lmax * d.n_kv_heads * d.head_dim * 4, kAlign);
+    w.total = o;
+    return w;
+}
+
+template <int D>
+pf_status set_attrs() {
+    cudaError_t e;
+    e = cudaFuncSetAttribute(pf::attn_fwd_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             pf::FwdCfg<D>::SMEM);
+    if (e != cudaSuccess) return PF_CUDA_ERROR;
+    e = cudaFuncSetAttribute(pf::attn_bwd_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             pf::BwdCfg<D>::SMEM);
+    if (e != cudaSuccess) return PF_CUDA_ERROR;
+    return PF_OK;
+}
+
+// ---- forward launch: queries [Lq] attend to prefix source [Lp] (all visible) + own causal keys
+template <int D>
+pf_status launch_fwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const pf_tensor& V1,
+                     int64_t Lp, const pf_tensor& K2, const pf_tensor& V2, const pf_tensor& O,
+                     float* LSE, int64_t lse_stride, int64_t Lq, cudaStream_t s) {
+    pf_ctx* ctx = g->ctx;
+    const int Hq = g->desc.n_q_heads, Hkv = g->desc.n_kv_heads;
+    CUtensorMap mQ, mK1, mV1, mK2, mV2;
+    pf_status st;
+    if ((st = make_map(ctx, &mQ, "Q", Q, Lq, Hq, D))) return st;
+    if ((st = make_map(ctx, &mK2, "K", K2, Lq, Hkv, D))) return st;
+    if ((st = make_map(ctx, &mV2, "V", V2, Lq, Hkv, D))) return st;
+    if (Lp > 0) {
+        if ((st = make_map(ctx, &mK1, "K1", K1, Lp, Hkv, D))) return st;
+        if ((st = make_map(ctx, &mV1, "V1", V1, Lp, Hkv, D))) return st;
+    } else {
+        mK1 = mK2;
+        mV1 = mV2;
+    }
+    pf::FwdParams p;
+    p.O = static_cast<__nv_bfloat16*>(O.ptr);
+    p.o_stride_tok = O.stride_tok;
+    p.o_stride_head = O.stride_head;
+    p.LSE = LSE;
+    p.lse_stride = lse_stride;
+    p.Lq = int(Lq);
+    p.Lp = int(Lp);
+    p.Hq = Hq;
+    p.Hkv = Hkv;
+    p.G = Hq / Hkv;
+    p.nRB = int((Lq + 127) / 128);
+    p.scale_log2 = g->sigma * 1.4426950408889634f;
+    const int nItems = p.nRB * p.G;
+    dim3 grid((nItems + 1) / 2, Hkv);
+    pf::attn_fwd_kernel<D><<<grid, pf::FwdCfg<D>::THREADS, pf::FwdCfg<D>::SMEM, s>>>(mQ, mK1, mV1, mK2,
+                                                                                 mV2, p);
+    PF_CUDA(ctx, cudaGetLastError());
+    return PF_OK;
+}
+
+int pick_parts(const pf_ctx* ctx, int G, int64_t n_tiles_times_hkv) {
+    if (ctx->bwd_head_parts > 0) return ctx->bwd_head_parts < G ? ctx->bwd_head_parts : G;
+    // heuristic: at least ~3 CTAs per SM of work items, but never more parts than heads
+    int parts = 1;
+    while (parts < G && n_tiles_times_hkv * parts < 3 * int64_t(ctx->num_sms)) ++parts;
+    return parts;
+}
+
+// ---- backward launch.  Keys of the prefix source accumulate into accK1/accV1 (fp32, +=),
+// keys of the causal source into accK2/accV2 (fp32, +=); dQ goes through the fp32 staging buffer
+// and is rounded to bf16 once all key tiles have contributed.
+template <int D>
+pf_status launch_bwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const pf_tensor& V1,
+                     int64_t Lp, const pf_tensor& K2, const pf_tensor& V2, const pf_tensor& O,
+                     const float* LSE, int64_t lse_stride, const pf_tensor& dO, float* accK1,
+                     float* accV1, float* accK2, float* accV2, const pf_tensor& dQ, int64_t Lq,
+                     cudaStream_t s) {
+    pf_ctx* ctx = g->ctx;
+    const int Hq = g->desc.n_q_heads, Hkv = g->desc.n_kv_heads, G = Hq / Hkv;
+    const WsLayout w = ws_layout(g->desc, Lq);
+    if (size_t(w.total) > g->ws_bytes)
+        return fail(ctx, PF_WORKSPACE, "workspace too small: need %lld bytes for %lld tokens, have %zu",
+                    (long long)w.total, (long long)Lq, g->ws_bytes);
+    float* lse2 = reinterpret_cast<float*>(g->ws + w.off_lse2);
+    float* delta = reinterpret_cast<float*>(g->ws + w.off_delta);
+    float* dqacc = reinterpret_cast<float*>(g->ws + w.off_dq);
+    const int Lpad = int(w.stat_stride);
+
+    CUtensorMap mQ, mdO, mK1, mV1, mK2, mV2;
+    pf_status st;
+    if ((st = make_map(ctx, &mQ, "Q", Q, Lq, Hq, D))) return st;
+    if ((st = make_map(ctx, &mdO, "dO", dO, Lq, Hq, D))) return st;
+    if ((st = make_map(ctx, &mK2, "K", K2, Lq, Hkv, D))) return st;
+    if ((st = make_map(ctx, &mV2, "V", V2, Lq, Hkv, D))) return st;
+    if (Lp > 0) {
+        if ((st = make_map(ctx, &mK1, "K1", K1, Lp, Hkv, D))) return st;
+        if ((st = make_map(ctx, &mV1, "V1", V1, Lp, Hkv, D))) return st;
+    } else {
+        mK1 = mK2;
+        mV1 = mV2;
+    }
+    PF_CUDA(ctx, cudaMemsetAsync(dqacc, 0, size_t(Lq) * Hq * D * 4, s));
+    {
+        const int64_t threads = int64_t(Lpad) * (D / 8);
+        dim3 grid(unsigned((threads + 255) / 256), Hq);
+        pf::bwd_preprocess_kernel<D><<<grid, 256, 0, s>>>(
+            static_cast<const __nv_bfloat16*>(O.ptr), O.stride_tok, O.stride_head,
+            static_cast<const __nv_bfloat16*>(dO.ptr), dO.stride_tok, dO.stride_head, LSE, lse_stride,
+            lse2, delta, w.stat_stride, int(Lq), Lpad);
+        PF_CUDA(ctx, cudaGetLastError());
+    }
+    pf::BwdParams p;
+    p.dQacc = dqacc;
+    p.accK1 = accK1; p.accV1 = accV1; p.accK2 = accK2; p.accV2 = accV2;
+    p.lse2 = lse2; p.delta = delta; p.stat_stride = w.stat_stride;
+    p.Lq = int(Lq); p.Lp = int(Lp);
+    p.Hq = Hq; p.Hkv = Hkv; p.G = G;
+    p.nQT = int((Lq + 127) / 128);
+    p.nPT = int((Lp + 127) / 128);
+    p.parts = pick_parts(ctx, G, int64_t(p.nQT + p.nPT) * Hkv);
+    p.hpp = (G + p.parts - 1) / p.parts;
+    p.scale_log2 = g->sigma * 1.4426950408889634f;
+    p.sigma = g->sigma;
+    const int64_t items = int64_t(p.nPT + p.nQT) * Hkv * p.parts;
+    pf::attn_bwd_kernel<D><<<unsigned(items), pf::BwdCfg<D>::THREADS, pf::BwdCfg<D>::SMEM, s>>>(
+        mQ, mdO, mK1, mV1, mK2, mV2, p);
+    PF_CUDA(ctx, cudaGetLastError());
+    {
+        const int64_t threads = Lq * Hq * (D / 8);
+        pf::acc_to_bf16_kernel<D><<<unsigned((threads + 255) / 256), 256, 0, s>>>(
+            dqacc, static_cast<__nv_bfloat16*>(dQ.ptr), dQ.stride_tok, dQ.stride_head, Lq, Hq,
+            g->sigma);
+        PF_CUDA(ctx, cudaGetLastError());
+    }
+    return PF_OK;
+}
+
+template <int D>
+pf_status launch_convert_kv(pf_group* g, const float* acc, const pf_tensor& dst, int64_t L,
+                            cudaStream_t s) {
+    const int Hkv = g->desc.n_kv_heads;
+    const int64_t threads = L * Hkv * (D / 8);
+    if (threads == 0) return PF_OK;
+    pf::acc_to_bf16_kernel<D><<<unsigned((threads + 255) / 256), 256, 0, s>>>(
+        acc, static_cast<__nv_bfloat16*>(dst.ptr), dst.stride_tok, dst.stride_head, L, Hkv, 1.0f);
+    PF_CUDA(g->ctx, cudaGetLastError());
+    return PF_OK;
+}
+
+pf_status check_cu(pf_ctx* ctx, int32_t n_seqs, const int32_t* cu) {
+    if (n_seqs < 0) return fail(ctx, PF_INVALID_ARG, "n_seqs < 0");
+    if (!cu) return fail(ctx, PF_INVALID_ARG, "cu_seqlens_host is NULL");
+    if (cu[0] != 0) return fail(ctx, PF_INVALID_ARG, "cu_seqlens_host[0] must be 0");
+    for (int i = 0; i < n_seqs; ++i)
+        if (cu[i + 1] < cu[i]) return fail(ctx, PF_INVALID_ARG, "cu_seqlens_host not monotone at %d", i);
+    return PF_OK;
+}
+
+inline pf_tensor tok_offset(const pf_tensor& t, int64_t tok) {
+    pf_tensor r = t;
+    r.ptr = static_cast<__nv_bfloat16*>(t.ptr) + tok * t.stride_tok;
+    return r;
+}
+
+}  // namespace
+
+// =================================================================================================
+// C ABI
+// =================================================================================================
+extern "C" {
+
+int32_t pf_version(void) { return 100; }
+
+pf_status pf_create(pf_ctx** out, int32_t device) {
+    if (!out) return PF_INVALID_ARG;
+    *out = nullptr;
+    pf_ctx* ctx = new (std::nothrow) pf_ctx();
+    if (!ctx) return PF_CUDA_ERROR;
+    ctx->device = device;
+    cudaError_t e = cudaSetDevice(device);
+    cudaDeviceProp prop;
+    if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, device);
+    if (e != cudaSuccess) {
+        delete ctx;
+        return PF_CUDA_ERROR;
+    }
+    if (prop.major != 10) {  // the kernels are sm_100a only: no fallback path exists
+        delete ctx;
+        return PF_UNSUPPORTED;
+    }
+    ctx->num_sms = prop.multiProcessorCount;
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q);
+    if (e != cudaSuccess || !fn || q != cudaDriverEntryPointSuccess) {
+        delete ctx;
+        return PF_CUDA_ERROR;
+    }
+    ctx->encode = reinterpret_cast<EncodeTiledFn>(fn);
+    if (set_attrs<64>() != PF_OK || set_attrs<128>() != PF_OK) {
+        delete ctx;
+        return PF_CUDA_ERROR;
+    }
+    *out = ctx;
+    return PF_OK;
+}
+
+pf_status pf_destroy(pf_ctx* ctx) {
+    if (!ctx) return PF_INVALID_ARG;
+    delete ctx;
+    return PF_OK;
+}
+
+const char* pf_last_error(const pf_ctx* ctx) { return ctx ? ctx->err : "pf_ctx is NULL"; }
+
+pf_status pf_set_option(pf_ctx* ctx, const char* name, int64_t value) {
+    if (!ctx || !name) return PF_INVALID_ARG;
+    if (strcmp(name, "bwd_head_parts") == 0) {
+        if (value < 0) return fail(ctx, PF_INVALID_ARG, "bwd_head_parts must be >= 0");
+        ctx->bwd_head_parts = int(value);
+        return PF_OK;
+    }
+    return fail(ctx, PF_INVALID_ARG, "unknown option '%s'", name);
+}
+
+size_t pf_workspace_bytes(const pf_desc* desc, int64_t Lp, int64_t max_Ls) {
+    if (!desc || Lp < 0 || max_Ls < 0 || desc->n_q_heads <= 0 || desc->n_kv_heads <= 0 ||
+        desc->head_dim <= 0)
+        return 0;
+    const int64_t Lmax = Lp > max_Ls ? Lp : max_Ls;
+    return size_t(ws_layout(*desc, Lmax).total) + size_t(kAlign);
+}
+
+pf_status pf_group_begin(pf_ctx* ctx, const pf_desc* desc, int64_t Lp, pf_tensor K1, pf_tensor V1,
+                         pf_tensor gK1, pf_tensor gV1, void* workspace, size_t workspace_bytes,
+                         void* stream, pf_group** out) {
+    if (!ctx) return PF_INVALID_ARG;
+    if (!out) return fail(ctx, PF_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    pf_status st;
+    if ((st = check_desc(ctx, desc))) return st;
+    if (Lp < 0 || Lp > (int64_t(1) << 30)) return fail(ctx, PF_INVALID_ARG, "Lp=%lld out of range", (long long)Lp);
+    const int Hkv = desc->n_kv_heads, d = desc->head_dim;
+    if ((st = check_tensor(ctx, "K1", K1, Lp, Hkv, d))) return st;
+    if ((st = check_tensor(ctx, "V1", V1, Lp, Hkv, d))) return st;
+    if ((gK1.ptr == nullptr) != (gV1.ptr == nullptr))
+        return fail(ctx, PF_INVALID_ARG, "gK1 and gV1 must both be given or both be NULL");
+    if (gK1.ptr) {
+        const pf_tensor* acc[2] = {&gK1, &gV1};
+        for (int i = 0; i < 2; ++i) {
+            if (reinterpret_cast<uintptr_t>(acc[i]->ptr) % 16 != 0)
+                return fail(ctx, PF_INVALID_ARG, "gK1/gV1 must be 16-byte aligned");
+            if (Lp > 0 && (acc[i]->stride_head != d || acc[i]->stride_tok != int64_t(Hkv) * d))
+                return fail(ctx, PF_UNSUPPORTED, "gK1/gV1 must be contiguous [Lp,Hkv,d] fp32");
+        }
+    }
+    if (!workspace || reinterpret_cast<uintptr_t>(workspace) % kAlign != 0)
+        return fail(ctx, PF_WORKSPACE, "workspace is NULL or not 256-byte aligned");
+    if (workspace_bytes < pf_workspace_bytes(desc, Lp, 0))
+        return fail(ctx, PF_WORKSPACE, "workspace of %zu bytes < pf_workspace_bytes = %zu",
+                    workspace_bytes, pf_workspace_bytes(desc, Lp, 0));
+    pf_group* g = new (std::nothrow) pf_group();
+    if (!g) return fail(ctx, PF_CUDA_ERROR, "out of host memory");
+    g->ctx = ctx;
+    g->desc = *desc;
+    g->sigma = desc->softmax_scale > 0.f ? desc->softmax_scale : 1.0f / sqrtf(float(d));
+    g->Lp = Lp;
+    g->K1 = K1;
+    g->V1 = V1;
+    g->gK1 = static_cast<float*>(gK1.ptr);
+    g->gV1 = static_cast<float*>(gV1.ptr);
+    g->ws = static_cast<uint8_t*>(workspace);
+    g->ws_bytes = workspace_bytes;
+    g->state = 0;
+    if (g->gK1 && Lp > 0) {
+        cudaStream_t s = static_cast<cudaStream_t>(stream);
+        const size_t bytes = size_t(Lp) * Hkv * d * 4;
+        cudaError_t e = cudaMemsetAsync(g->gK1, 0, bytes, s);
+        if (e == cudaSuccess) e = cudaMemsetAsync(g->gV1, 0, bytes, s);
+        if (e != cudaSuccess) {
+            delete g;
+            return fail(ctx, PF_CUDA_ERROR, "cudaMemsetAsync(gK1/gV1) failed: %s", cudaGetErrorString(e));
+        }
+    }
+    *out = g;
+    return PF_OK;
+}
+
+pf_status pf_group_end(pf_group* grp) {
+    if (!grp) return PF_INVALID_ARG;
+    delete grp;
+    return PF_OK;
+}
+
+pf_status pf_phaseA_fwd(pf_group* grp, pf_tensor Q1, pf_tensor O1, float* LSE1, void* stream) {
+    if (!grp) return PF_INVALID_ARG;
+    pf_ctx* ctx = grp->ctx;
+    if (grp->state != 0) return fail(ctx, PF_STATE, "pf_phaseA_fwd: Phase A already ran for this group");
+    const int Hq = grp->desc.n_q_heads, d = grp->desc.head_dim;
+    const int64_t Lp = grp->Lp;
+    pf_status st;
+    if ((st = check_tensor(ctx, "Q1", Q1, Lp, Hq, d))) return st;
+    if ((st = check_tensor(ctx, "O1", O1, Lp, Hq, d))) return st;
+    if (Lp > 0 && !LSE1) return fail(ctx, PF_INVALID_ARG, "LSE1 is NULL");
+    if (Lp > 0) {
+        cudaStream_t s = static_cast<cudaStream_t>(stream);
+        pf_tensor none = {nullptr, 0, 0};
+        st = d == 64 ? launch_fwd<64>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, Lp, s)
+                     : launch_fwd<128>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, Lp, s);
+        if (st) return st;
+    }
+    grp->state = 1;
+    return PF_OK;
+}
+
+pf_status pf_phaseB_fwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens_dev,
+                        const int32_t* cu_seqlens_host, pf_tensor Q2, pf_tensor K2, pf_tensor V2,
+                        pf_tensor O2, float* LSE2, void* stream) {
+    (void)cu_seqlens_dev;
+    if (!grp) return PF_INVALID_ARG;
+    pf_ctx* ctx = grp->ctx;
+    if (grp->state != 1) return fail(ctx, PF_STATE, "pf_phaseB_fwd needs Phase A done and Phase C not yet run");
+    pf_status st;
+    if ((st = check_cu(ctx, n_seqs, cu_seqlens_host))) return st;
+    const int Hq = grp->desc.n_q_heads, Hkv = grp->desc.n_kv_heads, d = grp->desc.head_dim;
+    const int64_t total = cu_seqlens_host[n_seqs];
+    if ((st = check_tensor(ctx, "Q2", Q2, total, Hq, d))) return st;
+    if ((st = check_tensor(ctx, "K2", K2, total, Hkv, d))) return st;
+    if ((st = check_tensor(ctx, "V2", V2, total, Hkv, d))) return st;
+    if ((st = check_tensor(ctx, "O2", O2, total, Hq, d))) return st;
+    if (total > 0 && !LSE2) return fail(ctx, PF_INVALID_ARG, "LSE2 is NULL");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    for (int i = 0; i < n_seqs; ++i) {
+        const int64_t t0 = cu_seqlens_host[i], Ls = cu_seqlens_host[i + 1] - t0;
+        if (Ls == 0) continue;
+        const pf_tensor q = tok_offset(Q2, t0), k = tok_offset(K2, t0), v = tok_offset(V2, t0),
+                        o = tok_offset(O2, t0);
+        st = d == 64 ? launch_fwd<64>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, Ls, s)
+                     : launch_fwd<128>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, Ls, s);
+        if (st) return st;
+    }
+    return PF_OK;
+}
+
+pf_status pf_phaseB_bwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens_dev,
+                        const int32_t* cu_seqlens_host, pf_tensor Q2, pf_tensor K2, pf_tensor V2,
+                        pf_tensor O2, const float* LSE2, pf_tensor dO2, pf_tensor dQ2,
+                        pf_tensor dK2, pf_tensor dV2, void* stream) {
+    (void)cu_seqlens_dev;
+    if (!grp) return PF_INVALID_ARG;
+    pf_ctx* ctx = grp->ctx;
+    if (grp->state != 1) return fail(ctx, PF_STATE, "pf_phaseB_bwd needs Phase A done and Phase C not yet run");
+    if (!grp->gK1 && grp->Lp > 0)
+        return fail(ctx, PF_STATE, "pf_phaseB_bwd: the group was opened without gK1/gV1");
+    pf_status st;
+    if ((st = check_cu(ctx, n_seqs, cu_seqlens_host))) return st;
+    const int Hq = grp->desc.n_q_heads, Hkv = grp->desc.n_kv_heads, d = grp->desc.head_dim;
+    const int64_t total = cu_seqlens_host[n_seqs];
+    if ((st = check_tensor(ctx, "Q2", Q2, total, Hq, d))) return st;
+    if ((st = check_tensor(ctx, "K2", K2, total, Hkv, d))) return st;
+    if ((st = check_tensor(ctx, "V2", V2, total, Hkv, d))) return st;
+    if ((st = check_tensor(ctx, "O2", O2, total, Hq, d))) return st;
+    if ((st = check_tensor(ctx, "dO2", dO2, total, Hq, d))) return st;
+    if ((st = check_tensor(ctx, "dQ2", dQ2, total, Hq, d))) return st;
+    if ((st = check_tensor(ctx, "dK2", dK2, total, Hkv, d))) return st;
+    if ((st = check_tensor(ctx, "dV2", dV2, total, Hkv, d))) return st;
+    if (total > 0 && !LSE2) return fail(ctx, PF_INVALID_ARG, "LSE2 is NULL");
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    for (int i = 0; i < n_seqs; ++i) {
+        const int64_t t0 = cu_seqlens_host[i], Ls = cu_seqlens_host[i + 1] - t0;
+        if (Ls == 0) continue;
+        const WsLayout w = ws_layout(grp->desc, Ls);
+        if (size_t(w.total) > grp->ws_bytes)
+            return fail(ctx, PF_WORKSPACE, "workspace too small for a suffix of %lld tokens", (long long)Ls);
+        float* ak = reinterpret_cast<float*>(grp->ws + w.off_ak);
+        float* av = reinterpret_cast<float*>(grp->ws + w.off_av);
+        const size_t kvb = size_t(Ls) * Hkv * d * 4;
+        PF_CUDA(ctx, cudaMemsetAsync(ak, 0, kvb, s));
+        PF_CUDA(ctx, cudaMemsetAsync(av, 0, kvb, s));
+        const pf_tensor q = tok_offset(Q2, t0), k = tok_offset(K2, t0), v = tok_offset(V2, t0),
+                        o = tok_offset(O2, t0), dout = tok_offset(dO2, t0), dq = tok_offset(dQ2, t0);
+        if (d == 64) {
+            st = launch_bwd<64>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, dout,
+                                grp->gK1, grp->gV1, ak, av, dq, Ls, s);
+            if (!st) st = launch_convert_kv<64>(grp, ak, tok_offset(dK2, t0), Ls, s);
+            if (!st) st = launch_convert_kv<64>(grp, av, tok_offset(dV2, t0), Ls, s);
+        } else {
+            st = launch_bwd<128>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, dout,
+                                 grp->gK1, grp->gV1, ak, av, dq, Ls, s);
+            if (!st) st = launch_convert_kv<128>(grp, ak, tok_offset(dK2, t0), Ls, s);
+            if (!st) st = launch_convert_kv<128>(grp, av, tok_offset(dV2, t0), Ls, s);
+        }
+        if (st) return st;
+    }
+    return PF_OK;
+}
+
+pf_status pf_phaseC_bwd(pf_group* grp, pf_tensor Q1, pf_tensor O1, const float* LSE1,
+                        pf_tensor dO1, pf_tensor dQ1, pf_tensor dK1, pf_tensor dV1, void* stream) {
+    if (!grp) return PF_INVALID_ARG;
+    pf_ctx* ctx = grp->ctx;
+    if (grp->state != 1) return fail(ctx, PF_STATE, "pf_phaseC_bwd needs Phase A done and runs once");
+    const int Hq = grp->desc.n_q_heads, Hkv = grp->desc.n_kv_heads, d = grp->desc.head_dim;
+    const int64_t Lp = grp->Lp;
+    pf_status st;
+    if ((st = check_tensor(ctx, "Q1", Q1, Lp, Hq, d))) return st;
+    if ((st = check_tensor(ctx, "O1", O1, Lp, Hq, d))) return st;
+    if ((st = check_tensor(ctx, "dO1", dO1, Lp, Hq, d))) return st;
+    if ((st = check_tensor(ctx, "dQ1", dQ1, Lp, Hq, d))) return st;
+    if ((st = check_tensor(ctx, "dK1", dK1, Lp, Hkv, d))) return st;
+    if ((st = check_tensor(ctx, "dV1", dV1, Lp, Hkv, d))) return st;
+    if (Lp > 0 && !LSE1) return fail(ctx, PF_INVALID_ARG, "LSE1 is NULL");
+    if (Lp > 0) {
+        cudaStream_t s = static_cast<cudaStream_t>(stream);
+        float* ak = grp->gK1;
+        float* av = grp->gV1;
+        if (!ak) {  // replay baseline: no injection, accumulate in the workspace
+            const WsLayout w = ws_layout(grp->desc, Lp);
+            if (size_t(w.total) > grp->ws_bytes) return fail(ctx, PF_WORKSPACE, "workspace too small");
+            ak = reinterpret_cast<float*>(grp->ws + w.off_ak);
+            av = reinterpret_cast<float*>(grp->ws + w.off_av);
+            const size_t kvb = size_t(Lp) * Hkv * d * 4;
+            PF_CUDA(ctx, cudaMemsetAsync(ak, 0, kvb, s));
+            PF_CUDA(ctx, cudaMemsetAsync(av, 0, kvb, s));
+        }
+        pf_tensor none = {nullptr, 0, 0};
+        if (d == 64) {
+            st = launch_bwd<64>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, dO1, nullptr,
+                                nullptr, ak, av, dQ1, Lp, s);
+            if (!st) st = launch_convert_kv<64>(grp, ak, dK1, Lp, s);
+            if (!st) st = launch_convert_kv<64>(grp, av, dV1, Lp, s);
+        } else {
+            st = launch_bwd<128>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, dO1, nullptr,
+                                 nullptr, ak, av, dQ1, Lp, s);
+            if (!st) st = launch_convert_kv<128>(grp, ak, dK1, Lp, s);
+            if (!st) st = launch_convert_kv<128>(grp, av, dV1, Lp, s);
+        }
+        if (st) return st;
+    }
+    grp->state = 2;
+    return PF_OK;
+}
+
+pf_status pf_offload(pf_ctx* ctx, const void* src_dev, void* dst_pinned_host, size_t bytes,
+                     void* side_stream) {
+    if (!ctx) return PF_INVALID_ARG;
+    if (bytes == 0) return PF_OK;
+    if (!src_dev || !dst_pinned_host) return fail(ctx, PF_INVALID_ARG, "pf_offload: NULL pointer");
+    PF_CUDA(ctx, cudaMemcpyAsync(dst_pinned_host, src_dev, bytes, cudaMemcpyDeviceToHost,
+                                 static_cast<cudaStream_t>(side_stream)));
+    return PF_OK;
+}
+
+pf_status pf_prefetch(pf_ctx* ctx, const void* src_pinned_host, void* dst_dev, size_t bytes,
+                      void* side_stream) {
+    if (!ctx) return PF_INVALID_ARG;
+    if (bytes == 0) return PF_OK;
+    if (!src_pinned_host || !dst_dev) return fail(ctx, PF_INVALID_ARG, "pf_prefetch: NULL pointer");
+    PF_CUDA(ctx, cudaMemcpyAsync(dst_dev, src_pinned_host, bytes, cudaMemcpyHostToDevice,
+                                 static_cast<cudaStream_t>(side_stream)));
+    return PF_OK;
+}
+
+}  // extern "C"

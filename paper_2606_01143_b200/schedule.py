@@ -1,0 +1,127 @@
+"""The three-phase call order of PAPER.md:148-160 on one GPU, and the N-times replay baseline.
+
+Host-side orchestration only: allocates device buffers with torch and issues the C-ABI calls of
+`binding` in the paper's order (Phase A once, Phase B fwd+bwd per suffix, Phase C once).  The
+replay baseline (BASELINE.json north_star item 3) runs the SAME kernels on each concatenated
+[P || S(i)]: a group opened with Lp = T_i and no gK1/gV1, `pf_phaseA_fwd` then `pf_phaseC_bwd`.
+"""
+from __future__ import annotations
+
+import dataclasses
+from typing import List, Optional, Sequence
+
+import torch
+
+from . import binding as pf
+
+
+@dataclasses.dataclass
+class DeviceGroup:
+    """Device-resident inputs and outputs of one rollout group (token-major [L, H, d])."""
+
+    Hq: int
+    Hkv: int
+    d: int
+    Lp: int
+    Ls: List[int]
+    Q1: torch.Tensor; K1: torch.Tensor; V1: torch.Tensor; dO1: torch.Tensor
+    Q2: List[torch.Tensor]; K2: List[torch.Tensor]; V2: List[torch.Tensor]; dO2: List[torch.Tensor]
+    # outputs
+    O1: torch.Tensor = None; LSE1: torch.Tensor = None
+    O2: List[torch.Tensor] = None; LSE2: List[torch.Tensor] = None
+    dQ2: List[torch.Tensor] = None; dK2: List[torch.Tensor] = None; dV2: List[torch.Tensor] = None
+    gK1: torch.Tensor = None; gV1: torch.Tensor = None
+    dQ1: torch.Tensor = None; dK1: torch.Tensor = None; dV1: torch.Tensor = None
+    workspace: torch.Tensor = None
+    desc: pf.pf_desc = None
+
+
+def to_device(inp, device="cuda", suffixes: Optional[Sequence[int]] = None) -> DeviceGroup:
+    """Copy a `inputs.GroupInputs` to the device and allocate every output buffer."""
+    s = inp.shape
+    idx = list(range(s.N)) if suffixes is None else list(suffixes)
+    dev = torch.device(device)
+    mv = lambda t: t.to(dev)
+    g = DeviceGroup(
+        s.n_q_heads, s.n_kv_heads, s.head_dim, s.Lp, [s.Ls[i] for i in idx],
+        mv(inp.Q1), mv(inp.K1), mv(inp.V1), mv(inp.dO1),
+        [mv(inp.Q2[i]) for i in idx], [mv(inp.K2[i]) for i in idx],
+        [mv(inp.V2[i]) for i in idx], [mv(inp.dO2[i]) for i in idx])
+    alloc_outputs(g)
+    return g
+
+
+def alloc_outputs(g: DeviceGroup) -> None:
+    dev = g.Q1.device
+    bf, f32 = torch.bfloat16, torch.float32
+    e = lambda L, H, dt=bf: torch.empty((L, H, g.d), dtype=dt, device=dev)
+    g.O1 = e(g.Lp, g.Hq); g.LSE1 = torch.empty((g.Hq, g.Lp), dtype=f32, device=dev)
+    g.O2 = [e(L, g.Hq) for L in g.Ls]
+    g.LSE2 = [torch.empty((g.Hq, L), dtype=f32, device=dev) for L in g.Ls]
+    g.dQ2 = [e(L, g.Hq) for L in g.Ls]
+    g.dK2 = [e(L, g.Hkv) for L in g.Ls]; g.dV2 = [e(L, g.Hkv) for L in g.Ls]
+    g.gK1 = e(g.Lp, g.Hkv, f32); g.gV1 = e(g.Lp, g.Hkv, f32)
+    g.dQ1 = e(g.Lp, g.Hq); g.dK1 = e(g.Lp, g.Hkv); g.dV1 = e(g.Lp, g.Hkv)
+    g.desc = pf.make_desc(g.Hq, g.Hkv, g.d)
+    nbytes = pf.pf_workspace_bytes(g.desc, g.Lp, max(g.Ls, default=0))
+    g.workspace = torch.empty(nbytes, dtype=torch.uint8, device=dev)
+
+
+def run_prefixflow_step(ctx, g: DeviceGroup, stream=None, after_each_suffix=None,
+                        order: Optional[Sequence[int]] = None) -> None:
+    """Phase A -> Phase B (fwd, bwd) per suffix -> Phase C."""
+    grp = pf.pf_group_begin(ctx, g.desc, g.Lp, g.K1, g.V1, g.gK1, g.gV1, g.workspace, stream)
+    try:
+        pf.pf_phaseA_fwd(grp, g.Q1, g.O1, g.LSE1, stream)
+        for i in (range(len(g.Ls)) if order is None else order):
+            cu = [0, g.Ls[i]]
+            pf.pf_phaseB_fwd(grp, cu, g.Q2[i], g.K2[i], g.V2[i], g.O2[i], g.LSE2[i], stream)
+            pf.pf_phaseB_bwd(grp, cu, g.Q2[i], g.K2[i], g.V2[i], g.O2[i], g.LSE2[i], g.dO2[i],
+                             g.dQ2[i], g.dK2[i], g.dV2[i], stream)
+            if after_each_suffix is not None:
+                after_each_suffix(i)
+        pf.pf_phaseC_bwd(grp, g.Q1, g.O1, g.LSE1, g.dO1, g.dQ1, g.dK1, g.dV1, stream)
+    finally:
+        pf.pf_group_end(grp)
+
+
+@dataclasses.dataclass
+class ReplayBuffers:
+    """Concatenated [P || S(i)] tensors of the N-times replay baseline (one set per trajectory)."""
+
+    T: List[int]
+    Q: List[torch.Tensor]; K: List[torch.Tensor]; V: List[torch.Tensor]; dO: List[torch.Tensor]
+    O: List[torch.Tensor]; LSE: List[torch.Tensor]
+    dQ: List[torch.Tensor]; dK: List[torch.Tensor]; dV: List[torch.Tensor]
+    workspace: torch.Tensor
+    desc: pf.pf_desc
+
+
+def make_replay(g: DeviceGroup, prefix_weight: Optional[float] = None) -> ReplayBuffers:
+    """Replay i sees dO = [w_i * dO1 ; dO2(i)], w_i = 1/N by default (reading 1)."""
+    n = len(g.Ls)
+    w = (1.0 / n if n else 1.0) if prefix_weight is None else prefix_weight
+    cat = lambda a, b: torch.cat([a, b], 0).contiguous()
+    Q = [cat(g.Q1, q) for q in g.Q2]; K = [cat(g.K1, k) for k in g.K2]
+    V = [cat(g.V1, v) for v in g.V2]
+    dO = [cat((g.dO1.float() * w).to(torch.bfloat16), x) for x in g.dO2]
+    T = [g.Lp + L for L in g.Ls]
+    dev = g.Q1.device
+    e = lambda L, H: torch.empty((L, H, g.d), dtype=torch.bfloat16, device=dev)
+    nbytes = pf.pf_workspace_bytes(g.desc, max(T, default=0), 0)
+    return ReplayBuffers(
+        T, Q, K, V, dO, [e(t, g.Hq) for t in T],
+        [torch.empty((g.Hq, t), dtype=torch.float32, device=dev) for t in T],
+        [e(t, g.Hq) for t in T], [e(t, g.Hkv) for t in T], [e(t, g.Hkv) for t in T],
+        torch.empty(nbytes, dtype=torch.uint8, device=dev), g.desc)
+
+
+def run_replay_step(ctx, r: ReplayBuffers, stream=None) -> None:
+    """N independent full-sequence causal fwd+bwd passes with the same kernels."""
+    for i, T in enumerate(r.T):
+        grp = pf.pf_group_begin(ctx, r.desc, T, r.K[i], r.V[i], None, None, r.workspace, stream)
+        try:
+            pf.pf_phaseA_fwd(grp, r.Q[i], r.O[i], r.LSE[i], stream)
+            pf.pf_phaseC_bwd(grp, r.Q[i], r.O[i], r.LSE[i], r.dO[i], r.dQ[i], r.dK[i], r.dV[i], stream)
+        finally:
+            pf.pf_group_end(grp)

@@ -1,0 +1,206 @@
+"""GPU parity: every C-ABI call vs the fp64 oracle, element by element, on the same seeded inputs.
+
+All tests here need a B200 (`-m gpu`) and go through the C ABI via the ctypes binding.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2606_01143_b200 import binding as pf
+from paper_2606_01143_b200 import inputs, schedule
+from parity_util import check, compare_group
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    c = pf.pf_create(0)
+    yield c
+    pf.pf_destroy(c)
+
+
+def run_and_compare(ctx, shape, weights=None, order=None, zero_dO1=False, parts=None):
+    inp = inputs.make_group(shape)
+    if zero_dO1:
+        inp.dO1.zero_()
+    ref = oracle.group_reference(inp, weights=weights, order=order)
+    g = schedule.to_device(inp)
+    snaps = {}
+
+    def snap(i):
+        snaps[i] = (g.gK1.clone(), g.gV1.clone())
+
+    if parts is not None:
+        pf.pf_set_option(ctx, "bwd_head_parts", parts)
+    try:
+        schedule.run_prefixflow_step(ctx, g, after_each_suffix=snap, order=order)
+        torch.cuda.synchronize()
+    finally:
+        if parts is not None:
+            pf.pf_set_option(ctx, "bwd_head_parts", 0)
+    return g, ref, compare_group(g, ref, snaps)
+
+
+def test_config_tiny(ctx):
+    """BASELINE.json configs[0]: 2q/2kv, d=64, Lp=256, N=4 x 64, seed 0."""
+    run_and_compare(ctx, inputs.config_tiny())
+
+
+def test_config_tiny_unit_logits(ctx):
+    """Same shapes, unit-logit distribution (online-softmax rescaling is exercised)."""
+    run_and_compare(ctx, inputs.config_tiny(dist="unit"))
+
+
+@pytest.mark.parametrize("Hq,Hkv,d,Lp,Ls", [
+    (4, 1, 128, 300, [129, 64]),       # GQA 4:1, ragged prefix tail, suffix spanning 2 tiles
+    (7, 1, 128, 129, [65, 1, 300]),    # GQA 7:1, Lp one past a tile, Ls = 1
+    (2, 2, 64, 127, [63, 127]),        # d = 64, everything one short of a tile
+    (4, 2, 64, 128, [128, 200]),       # exact tiles
+    (2, 1, 128, 1000, [257]),          # several prefix tiles
+    (1, 1, 128, 1, [1]),               # smallest non-empty
+])
+@pytest.mark.parametrize("dist", ["std", "unit"])
+def test_shapes(ctx, Hq, Hkv, d, Lp, Ls, dist):
+    run_and_compare(ctx, inputs.small_case(Hq, Hkv, d, Lp, Ls, seed=11, dist=dist))
+
+
+@pytest.mark.parametrize("parts", [1, 2, 7])
+def test_bwd_head_parts(ctx, parts):
+    """gK1/gV1 accumulation with the KV tile owned by one CTA (no contention) or split over heads."""
+    run_and_compare(ctx, inputs.small_case(7, 1, 128, 260, [140, 70], seed=5, dist="unit"), parts=parts)
+
+
+def test_degenerate_lengths(ctx):
+    """Ls = 0 is a no-op; Lp = 0 makes Phase B plain causal attention (SURVEY.md §8c reading 17)."""
+    run_and_compare(ctx, inputs.small_case(2, 1, 64, 200, [0, 70], seed=3))
+    run_and_compare(ctx, inputs.small_case(2, 1, 64, 0, [70, 130], seed=4))
+
+
+def test_n1_equals_full_pass(ctx):
+    run_and_compare(ctx, inputs.small_case(4, 2, 128, 150, [90], seed=9, dist="unit"))
+
+
+def test_pure_coupling_zero_dO1(ctx):
+    """dO1 = 0 (suffix-only loss, top layer): dQ1 = 0, dK1 = gK1, dV1 = gV1 (reading 1)."""
+    g, ref, _ = run_and_compare(ctx, inputs.small_case(4, 2, 64, 200, [100, 60], seed=2, dist="unit"),
+                                zero_dO1=True)
+    assert float(g.dQ1.float().abs().max()) == 0.0
+
+
+def test_suffix_order_permuted(ctx):
+    """Organisation independence: suffix order only changes fp32 rounding."""
+    shape = inputs.small_case(4, 2, 128, 260, [100, 140, 33], seed=21, dist="unit")
+    g0, ref, _ = run_and_compare(ctx, shape)
+    g1, _, _ = run_and_compare(ctx, shape, order=[2, 0, 1])
+    check("dK1 permuted vs natural order", g1.dK1, g0.dK1.double().cpu().numpy())
+    check("dV1 permuted vs natural order", g1.dV1, g0.dV1.double().cpu().numpy())
+
+
+def test_nonzero_preexisting_accumulator_is_zeroed(ctx):
+    """pf_group_begin zeroes gK1/gV1 (no state is reused across groups)."""
+    shape = inputs.small_case(2, 1, 64, 130, [70], seed=8)
+    inp = inputs.make_group(shape)
+    ref = oracle.group_reference(inp)
+    g = schedule.to_device(inp)
+    g.gK1.fill_(123.0); g.gV1.fill_(-7.0)
+    snaps = {}
+    schedule.run_prefixflow_step(ctx, g, after_each_suffix=lambda i: snaps.update(
+        {i: (g.gK1.clone(), g.gV1.clone())}))
+    torch.cuda.synchronize()
+    compare_group(g, ref, snaps)
+
+
+def test_strided_inputs(ctx):
+    """Non-contiguous token / head strides (packed QKV projection output layout)."""
+    shape = inputs.small_case(4, 2, 64, 140, [75], seed=13, dist="unit")
+    inp = inputs.make_group(shape)
+    ref = oracle.group_reference(inp)
+    g = schedule.to_device(inp)
+    Hq, Hkv, d = 4, 2, 64
+    # Q, K, V as slices of one fused [L, Hq + 2 Hkv, d] buffer
+    def fuse(q, k, v):
+        buf = torch.empty((q.shape[0], Hq + 2 * Hkv, d), dtype=torch.bfloat16, device=q.device)
+        buf[:, :Hq] = q; buf[:, Hq:Hq + Hkv] = k; buf[:, Hq + Hkv:] = v
+        return buf[:, :Hq], buf[:, Hq:Hq + Hkv], buf[:, Hq + Hkv:]
+    g.Q1, g.K1, g.V1 = fuse(g.Q1, g.K1, g.V1)
+    g.Q2[0], g.K2[0], g.V2[0] = fuse(g.Q2[0], g.K2[0], g.V2[0])
+    assert not g.Q1.is_contiguous()
+    schedule.run_prefixflow_step(ctx, g)
+    torch.cuda.synchronize()
+    compare_group(g, ref)
+
+
+def test_replay_baseline_matches_oracle(ctx):
+    """The N-times replay (same kernels on [P||S(i)]) reproduces each full-sequence oracle pass."""
+    shape = inputs.small_case(4, 2, 128, 200, [90, 150], seed=17, dist="unit")
+    inp = inputs.make_group(shape)
+    ref = oracle.group_reference(inp)           # replay i uses prefix adjoint dO1 / N
+    g = schedule.to_device(inp)
+    r = schedule.make_replay(g)
+    schedule.run_replay_step(ctx, r)
+    torch.cuda.synchronize()
+    Lp = shape.Lp
+    for i in range(shape.N):
+        rep = ref.replay[i]
+        check(f"replay O[{i}]", r.O[i], rep["o"])
+        check(f"replay LSE[{i}]", r.LSE[i], rep["lse"], lse=True)
+        check(f"replay dQ[{i}]", r.dQ[i], rep["dq"])
+        dk = rep["dk"].copy(); dv = rep["dv"].copy()
+        dk[:Lp] += rep["gk"]; dv[:Lp] += rep["gv"]
+        check(f"replay dK[{i}]", r.dK[i], dk)
+        check(f"replay dV[{i}]", r.dV[i], dv)
+
+
+def test_two_groups_on_two_streams(ctx):
+    """No hidden shared state: two groups interleaved on two streams both match."""
+    shapes = [inputs.small_case(2, 1, 64, 150, [60], seed=31), inputs.small_case(4, 4, 128, 90, [140], seed=32)]
+    inps = [inputs.make_group(s) for s in shapes]
+    refs = [oracle.group_reference(i) for i in inps]
+    gs = [schedule.to_device(i) for i in inps]
+    torch.cuda.synchronize()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    for g, s in zip(gs, streams):
+        with torch.cuda.stream(s):
+            schedule.run_prefixflow_step(ctx, g, stream=s)
+    torch.cuda.synchronize()
+    for g, ref in zip(gs, refs):
+        compare_group(g, ref)
+
+
+def test_error_paths(ctx):
+    """Validation returns a status without launching."""
+    dev = "cuda"
+    bf = torch.bfloat16
+    K = torch.zeros((128, 2, 64), dtype=bf, device=dev)
+    gk = torch.zeros((128, 2, 64), dtype=torch.float32, device=dev)
+    ws = torch.empty(pf.pf_workspace_bytes(pf.make_desc(4, 2, 64), 128, 128), dtype=torch.uint8, device=dev)
+    with pytest.raises(pf.PrefixFlowError) as e:
+        pf.pf_group_begin(ctx, pf.make_desc(3, 2, 64), 128, K, K, gk, gk, ws)
+    assert e.value.status == pf.PF_INVALID_ARG
+    with pytest.raises(pf.PrefixFlowError) as e:
+        pf.pf_group_begin(ctx, pf.make_desc(4, 2, 96), 128, K, K, gk, gk, ws)
+    assert e.value.status == pf.PF_UNSUPPORTED
+    with pytest.raises(pf.PrefixFlowError) as e:
+        pf.pf_group_begin(ctx, pf.make_desc(4, 2, 64), 128, K, K, gk, gk, ws[:1024])
+    assert e.value.status == pf.PF_WORKSPACE
+    with pytest.raises(pf.PrefixFlowError) as e:   # misaligned base pointer
+        pf.pf_group_begin(ctx, pf.make_desc(4, 2, 64), 100, K.view(-1)[4:4 + 100 * 128].view(100, 2, 64),
+                          K, gk, gk, ws)
+    assert e.value.status == pf.PF_INVALID_ARG
+    grp = pf.pf_group_begin(ctx, pf.make_desc(4, 2, 64), 128, K, K, gk, gk, ws)
+    Q = torch.zeros((128, 4, 64), dtype=bf, device=dev)
+    lse = torch.zeros((4, 128), dtype=torch.float32, device=dev)
+    with pytest.raises(pf.PrefixFlowError) as e:   # Phase C before Phase A
+        pf.pf_phaseC_bwd(grp, Q, Q, lse, Q, Q, K, K)
+    assert e.value.status == pf.PF_STATE
+    with pytest.raises(pf.PrefixFlowError) as e:   # Phase B before Phase A
+        pf.pf_phaseB_fwd(grp, [0, 128], Q, K, K, Q, lse)
+    assert e.value.status == pf.PF_STATE
+    pf.pf_phaseA_fwd(grp, Q, Q.clone(), lse)
+    with pytest.raises(pf.PrefixFlowError) as e:   # non-monotone cu_seqlens
+        pf.pf_phaseB_fwd(grp, [0, 64, 32], Q, K, K, Q, lse)
+    assert e.value.status == pf.PF_INVALID_ARG
+    pf.pf_group_end(grp)
+    torch.cuda.synchronize()
