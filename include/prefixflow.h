@@ -76,6 +76,20 @@ const char* pf_last_error(const pf_ctx* ctx);
  *                      (gK1/gV1 += without contention), G = maximal parallelism, most atomics. */
 pf_status pf_set_option(pf_ctx* ctx, const char* name, int64_t value);
 
+/*   "profile"        : 1 = bracket every attention kernel launch (not the elementwise helpers)
+ *                      with a pair of CUDA events on the launch stream; read with pf_profile_read.
+ *                      Used by bench.py for the roofline of the dominant kernel.  0 = off. */
+
+/* Number of kernels this context has launched so far ("kernel_launches"), or -1 for an unknown
+ * counter name.  Host-side bookkeeping only. */
+int64_t pf_counter(const pf_ctx* ctx, const char* name);
+
+/* Profiling read-out (needs option "profile" = 1).  kind: 0 = attention forward kernel,
+ * 1 = attention backward kernel.  Synchronises on the recorded events, adds up their durations,
+ * writes the number of launches and the total milliseconds since the previous read of that kind,
+ * and recycles the events. */
+pf_status pf_profile_read(pf_ctx* ctx, int32_t kind, int64_t* launches, double* total_ms);
+
 /* Bytes of caller-provided scratch needed by a group with prefix length Lp whose longest Phase-B
  * call carries max_Ls suffix tokens (fp32 dQ / dK2 / dV2 staging and softmax statistics). */
 size_t pf_workspace_bytes(const pf_desc* desc, int64_t Lp, int64_t max_Ls);

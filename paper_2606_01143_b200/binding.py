@@ -23,7 +23,8 @@ STATUS_NAMES = {0: "PF_OK", 1: "PF_INVALID_ARG", 2: "PF_UNSUPPORTED", 3: "PF_CUD
 # every symbol include/prefixflow.h declares
 SYMBOLS = ("pf_version", "pf_create", "pf_destroy", "pf_last_error", "pf_set_option",
            "pf_workspace_bytes", "pf_group_begin", "pf_phaseA_fwd", "pf_phaseB_fwd",
-           "pf_phaseB_bwd", "pf_phaseC_bwd", "pf_group_end", "pf_offload", "pf_prefetch")
+           "pf_phaseB_bwd", "pf_phaseC_bwd", "pf_group_end", "pf_offload", "pf_prefetch",
+           "pf_counter", "pf_profile_read")
 
 
 class PrefixFlowError(RuntimeError):
@@ -67,6 +68,11 @@ def lib() -> ctypes.CDLL:
     L.pf_last_error.argtypes = [vp]
     L.pf_set_option.restype = i32
     L.pf_set_option.argtypes = [vp, ctypes.c_char_p, i64]
+    L.pf_counter.restype = i64
+    L.pf_counter.argtypes = [vp, ctypes.c_char_p]
+    L.pf_profile_read.restype = i32
+    L.pf_profile_read.argtypes = [vp, i32, ctypes.POINTER(ctypes.c_int64),
+                                  ctypes.POINTER(ctypes.c_double)]
     L.pf_workspace_bytes.restype = ctypes.c_size_t
     L.pf_workspace_bytes.argtypes = [ctypes.POINTER(pf_desc), i64, i64]
     L.pf_group_begin.restype = i32
@@ -167,6 +173,17 @@ def pf_last_error(ctx: _Handle) -> str:
 
 def pf_set_option(ctx: _Handle, name: str, value: int) -> None:
     _check(lib().pf_set_option(ctx.ptr, name.encode(), int(value)), ctx)
+
+
+def pf_counter(ctx: _Handle, name: str) -> int:
+    return int(lib().pf_counter(ctx.ptr, name.encode()))
+
+
+def pf_profile_read(ctx: _Handle, kind: int):
+    """(launches, total_ms) of the attention kernels of `kind` (0 fwd, 1 bwd) since the last read."""
+    n, ms = ctypes.c_int64(), ctypes.c_double()
+    _check(lib().pf_profile_read(ctx.ptr, int(kind), ctypes.byref(n), ctypes.byref(ms)), ctx)
+    return int(n.value), float(ms.value)
 
 
 def pf_workspace_bytes(desc: pf_desc, Lp: int, max_Ls: int) -> int:

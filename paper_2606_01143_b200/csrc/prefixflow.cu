@@ -8,6 +8,7 @@
 #include <cstring>
 #include <cmath>
 #include <new>
+#include <vector>
 
 #include "../../include/prefixflow.h"
 #include "attn_fwd.cuh"
@@ -26,12 +27,20 @@ inline int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
 
 }  // namespace
 
+struct ProfRec {
+    cudaEvent_t a, b;
+    int kind;
+};
+
 struct pf_ctx {
     int device = 0;
     int num_sms = 0;
     EncodeTiledFn encode = nullptr;
     int bwd_head_parts = 0;  // 0 = heuristic
-    bool attr_set = false;
+    bool profile = false;
+    int64_t n_launches = 0;
+    std::vector<ProfRec> prof;         // recorded, not yet read
+    std::vector<cudaEvent_t> ev_pool;  // recycled events
     char err[512] = {0};
 };
 
@@ -66,6 +75,36 @@ pf_status fail(pf_ctx* ctx, pf_status st, const char* fmt, ...) {
         if (e_ != cudaSuccess)                                                          \
             return fail(ctx, PF_CUDA_ERROR, "%s failed: %s", #call, cudaGetErrorString(e_)); \
     } while (0)
+
+cudaEvent_t prof_event(pf_ctx* ctx) {
+    cudaEvent_t e = nullptr;
+    if (!ctx->ev_pool.empty()) {
+        e = ctx->ev_pool.back();
+        ctx->ev_pool.pop_back();
+    } else if (cudaEventCreate(&e) != cudaSuccess) {
+        e = nullptr;
+    }
+    return e;
+}
+
+// RAII bracket: records an event pair around one attention kernel launch when profiling is on
+struct ProfScope {
+    pf_ctx* ctx;
+    cudaStream_t s;
+    ProfRec r{nullptr, nullptr, 0};
+    ProfScope(pf_ctx* c, int kind, cudaStream_t st) : ctx(c), s(st) {
+        if (!ctx->profile) return;
+        r.kind = kind;
+        r.a = prof_event(ctx);
+        r.b = prof_event(ctx);
+        if (r.a) cudaEventRecord(r.a, s);
+    }
+    ~ProfScope() {
+        if (!ctx->profile || !r.a || !r.b) return;
+        cudaEventRecord(r.b, s);
+        ctx->prof.push_back(r);
+    }
+};
 
 pf_status check_desc(pf_ctx* ctx, const pf_desc* d) {
     if (!d) return fail(ctx, PF_INVALID_ARG, "desc is NULL");
@@ -183,9 +222,13 @@ pf_status launch_fwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const
     p.scale_log2 = g->sigma * 1.4426950408889634f;
     const int nItems = p.nRB * p.G;
     dim3 grid((nItems + 1) / 2, Hkv);
-    pf::attn_fwd_kernel<D><<<grid, pf::FwdCfg<D>::THREADS, pf::FwdCfg<D>::SMEM, s>>>(mQ, mK1, mV1, mK2,
-                                                                                 mV2, p);
+    {
+        ProfScope prof(ctx, 0, s);
+        pf::attn_fwd_kernel<D><<<grid, pf::FwdCfg<D>::THREADS, pf::FwdCfg<D>::SMEM, s>>>(
+            mQ, mK1, mV1, mK2, mV2, p);
+    }
     PF_CUDA(ctx, cudaGetLastError());
+    ctx->n_launches += 1;
     return PF_OK;
 }
 
@@ -239,6 +282,7 @@ pf_status launch_bwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const
             static_cast<const __nv_bfloat16*>(dO.ptr), dO.stride_tok, dO.stride_head, LSE, lse_stride,
             lse2, delta, w.stat_stride, int(Lq), Lpad);
         PF_CUDA(ctx, cudaGetLastError());
+        ctx->n_launches += 1;
     }
     pf::BwdParams p;
     p.dQacc = dqacc;
@@ -253,15 +297,20 @@ pf_status launch_bwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const
     p.scale_log2 = g->sigma * 1.4426950408889634f;
     p.sigma = g->sigma;
     const int64_t items = int64_t(p.nPT + p.nQT) * Hkv * p.parts;
-    pf::attn_bwd_kernel<D><<<unsigned(items), pf::BwdCfg<D>::THREADS, pf::BwdCfg<D>::SMEM, s>>>(
-        mQ, mdO, mK1, mV1, mK2, mV2, p);
+    {
+        ProfScope prof(ctx, 1, s);
+        pf::attn_bwd_kernel<D><<<unsigned(items), pf::BwdCfg<D>::THREADS, pf::BwdCfg<D>::SMEM, s>>>(
+            mQ, mdO, mK1, mV1, mK2, mV2, p);
+    }
     PF_CUDA(ctx, cudaGetLastError());
+    ctx->n_launches += 1;
     {
         const int64_t threads = Lq * Hq * (D / 8);
         pf::acc_to_bf16_kernel<D><<<unsigned((threads + 255) / 256), 256, 0, s>>>(
             dqacc, static_cast<__nv_bfloat16*>(dQ.ptr), dQ.stride_tok, dQ.stride_head, Lq, Hq,
             g->sigma);
         PF_CUDA(ctx, cudaGetLastError());
+        ctx->n_launches += 1;
     }
     return PF_OK;
 }
@@ -275,6 +324,7 @@ pf_status launch_convert_kv(pf_group* g, const float* acc, const pf_tensor& dst,
     pf::acc_to_bf16_kernel<D><<<unsigned((threads + 255) / 256), 256, 0, s>>>(
         acc, static_cast<__nv_bfloat16*>(dst.ptr), dst.stride_tok, dst.stride_head, L, Hkv, 1.0f);
     PF_CUDA(g->ctx, cudaGetLastError());
+    g->ctx->n_launches += 1;
     return PF_OK;
 }
 
@@ -338,6 +388,11 @@ pf_status pf_create(pf_ctx** out, int32_t device) {
 
 pf_status pf_destroy(pf_ctx* ctx) {
     if (!ctx) return PF_INVALID_ARG;
+    for (auto& r : ctx->prof) {
+        cudaEventDestroy(r.a);
+        cudaEventDestroy(r.b);
+    }
+    for (auto e : ctx->ev_pool) cudaEventDestroy(e);
     delete ctx;
     return PF_OK;
 }
@@ -351,7 +406,42 @@ pf_status pf_set_option(pf_ctx* ctx, const char* name, int64_t value) {
         ctx->bwd_head_parts = int(value);
         return PF_OK;
     }
+    if (strcmp(name, "profile") == 0) {
+        ctx->profile = value != 0;
+        return PF_OK;
+    }
     return fail(ctx, PF_INVALID_ARG, "unknown option '%s'", name);
+}
+
+int64_t pf_counter(const pf_ctx* ctx, const char* name) {
+    if (!ctx || !name) return -1;
+    if (strcmp(name, "kernel_launches") == 0) return ctx->n_launches;
+    return -1;
+}
+
+pf_status pf_profile_read(pf_ctx* ctx, int32_t kind, int64_t* launches, double* total_ms) {
+    if (!ctx) return PF_INVALID_ARG;
+    if (!launches || !total_ms) return fail(ctx, PF_INVALID_ARG, "pf_profile_read: NULL output");
+    int64_t n = 0;
+    double ms = 0.0;
+    std::vector<ProfRec> keep;
+    for (auto& r : ctx->prof) {
+        if (r.kind != kind) {
+            keep.push_back(r);
+            continue;
+        }
+        PF_CUDA(ctx, cudaEventSynchronize(r.b));
+        float t = 0.f;
+        PF_CUDA(ctx, cudaEventElapsedTime(&t, r.a, r.b));
+        ms += t;
+        n += 1;
+        ctx->ev_pool.push_back(r.a);
+        ctx->ev_pool.push_back(r.b);
+    }
+    ctx->prof.swap(keep);
+    *launches = n;
+    *total_ms = ms;
+    return PF_OK;
 }
 
 size_t pf_workspace_bytes(const pf_desc* desc, int64_t Lp, int64_t max_Ls) {
