@@ -1,0 +1,423 @@
+#!/usr/bin/env python
+"""bench.py -- one B200 (or N independent ranks): the A -> B(xN) -> C attention step of PrefixFlow's
+training-time KV cache through the C ABI, against the build's own N-times replay baseline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 7b|ragged|32k|sweep-rR-nN|tiny]
+    python bench.py --impl reference ...      # times the fp64 CPU oracle on a bounded sample
+
+A "step" is one pass of the whole hot path over one synthetic rollout group (SURVEY.md §8a rows
+a1-a4): pf_group_begin, pf_phaseA_fwd, N x (pf_phaseB_fwd, pf_phaseB_bwd), pf_phaseC_bwd.
+Prints ONE JSON line (rank 0).  Keys follow the driver's contract; DESIGN.md "Measurement" explains
+every number.  Nothing here reads /root/reference; every input is seeded and synthetic
+(paper_2606_01143_b200/inputs.py).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = ("A+B+C attention step throughput (algorithmic TFLOP/s; step time vs N-times replay and "
+          "Phase-B TFLOP/s / % of BF16 peak in extra keys)")
+UNIT = "TFLOP/s"
+L2_BYTES = 126 * 2 ** 20
+
+
+# --------------------------------------------------------------------------------------------------
+# algorithmic work (fwd = 4 d pairs Hq, bwd = 10 d pairs Hq; tile padding not counted)
+# --------------------------------------------------------------------------------------------------
+def tri(L: int) -> int:
+    return L * (L + 1) // 2
+
+
+def flops(shape) -> dict:
+    Hq, d, Lp = shape.n_q_heads, shape.head_dim, shape.Lp
+    pa = tri(Lp)
+    pb = [Ls * Lp + tri(Ls) for Ls in shape.Ls]
+    pr = [tri(Lp + Ls) for Ls in shape.Ls]
+    f = dict(A=4 * d * pa * Hq, B_fwd=4 * d * sum(pb) * Hq, B_bwd=10 * d * sum(pb) * Hq,
+             C=10 * d * pa * Hq, replay=14 * d * sum(pr) * Hq)
+    f["B_bwd_each"] = [10 * d * p * Hq for p in pb]
+    f["B_fwd_each"] = [4 * d * p * Hq for p in pb]
+    f["step"] = f["A"] + f["B_fwd"] + f["B_bwd"] + f["C"]
+    f["ideal_speedup"] = sum(pr) / (pa + sum(pb)) if (pa + sum(pb)) else 1.0
+    return f
+
+
+def pick_config(name: str):
+    from paper_2606_01143_b200 import inputs
+    if name == "7b":
+        return inputs.config_7b()
+    if name == "tiny":
+        return inputs.config_tiny()
+    if name == "ragged":
+        return inputs.config_ragged()
+    if name == "32k":
+        return inputs.config_32k()
+    if name.startswith("sweep-r"):
+        r, n = name[len("sweep-r"):].split("-n")
+        return inputs.config_sweep(int(r), int(n))
+    raise SystemExit(f"unknown --config {name}")
+
+
+def measured_peaks() -> dict:
+    """MEASURED_PEAKS.json (driver-written) or the fallback of /opt/skills/guides/B200_PROFILING.md."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            m = json.load(f)
+        return dict(burst=float(m["bf16_tflops"]), sustained=float(m["bf16_tflops_sustained"]),
+                    hbm=float(m["hbm_gbs"]), source="measured (MEASURED_PEAKS.json)")
+    return dict(burst=1590.0, sustained=1400.0, hbm=6650.0, source="fallback (B200_PROFILING.md)")
+
+
+def ncu_traffic(kernel: str, config: str):
+    """dram bytes per launch of `kernel` from the committed ncu --set full summary, else None."""
+    p = os.path.join(ROOT, "profiles", "roofline_traffic.csv")
+    if not os.path.exists(p):
+        return None
+    with open(p) as f:
+        for line in f:
+            parts = [x.strip() for x in line.split(",")]
+            if len(parts) >= 3 and parts[0] == kernel and parts[1] == config:
+                try:
+                    return float(parts[2])
+                except ValueError:
+                    return None
+    return None
+
+
+# --------------------------------------------------------------------------------------------------
+# clocks sampled DURING the timed region (NVML in a thread; nvidia-smi's own start-up is too slow)
+# --------------------------------------------------------------------------------------------------
+class ClockSampler:
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown",
+               0x4: "sw_power_cap", 0x80: "hw_power_brake", 0x2: "applications_clocks_setting"}
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.power = [], set(), []
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:  # NVML missing: clocks are reported as null
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                for bit, name in self.REASONS.items():
+                    if r & bit:
+                        self.reasons.add(name)
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+            except Exception:
+                pass
+            time.sleep(0.005)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self) -> dict:
+        if not self.samples:
+            return dict(sm_mhz=None, sm_max_mhz=self.max_mhz, reasons=[], samples=0)
+        return dict(sm_mhz=statistics.median(self.samples), sm_max_mhz=self.max_mhz,
+                    reasons=sorted(self.reasons), samples=len(self.samples),
+                    power_w_max=max(self.power) if self.power else None)
+
+
+# --------------------------------------------------------------------------------------------------
+# CPU oracle leg (cpu_baseline and --impl reference): a BOUNDED sample of the same workload
+# --------------------------------------------------------------------------------------------------
+def oracle_sample(shape, budget_flops: float = 6e11):
+    """Phase B forward + backward of (suffix i, KV head g) units -- the G query heads of g: every
+    suffix row (O2, LSE2, delta, dQ2) and every key column (gK1/gV1 of the prefix keys, dK2/dV2
+    of the suffix keys) -- as many whole units as fit `budget_flops` algorithmic flops (at least
+    one; if one unit alone exceeds the budget its key columns are strided).  Returns
+    (seconds, algorithmic flops of what was computed, description, threads)."""
+    import numpy as np
+    import oracle
+    from paper_2606_01143_b200 import inputs
+    d, G, Lp = shape.head_dim, shape.G, shape.Lp
+    units = [(i, g) for i in range(shape.N) for g in range(shape.n_kv_heads)]
+    # algorithmic count 14 d per (query, key) pair and head: the row side covers S, PV, dP, dQ (8 d),
+    # the column side the S recompute, dK, dV (6 d); the oracle's own extra dP recompute is not counted
+    unit_flops = lambda i: 14 * d * (shape.Ls[i] * Lp + tri(shape.Ls[i])) * G
+    chosen, acc = [], 0.0
+    for (i, g) in units:
+        if chosen and acc + unit_flops(i) > budget_flops:
+            break
+        chosen.append((i, g))
+        acc += unit_flops(i)
+    stride = 1
+    if len(chosen) == 1:
+        i = chosen[0][0]
+        pairs = shape.Ls[i] * Lp + tri(shape.Ls[i])
+        while 8 * d * pairs * G + 6 * d * pairs * G / stride > budget_flops and stride < 64:
+            stride *= 2
+    inp = inputs.make_group(shape, only_suffixes=sorted({i for i, _ in chosen}))
+    done, dt = 0.0, 0.0
+    for (i, g) in chosen:
+        Ls = shape.Ls[i]
+        pj = np.arange(0, Lp, stride, dtype=np.int64)
+        sj = np.arange(0, Ls, stride, dtype=np.int64)
+        t0 = time.perf_counter()
+        oracle.sampled_phaseB(inp, i, g, pj, sj)
+        dt += time.perf_counter() - t0
+        col_pairs = int(len(pj) * Ls + sum(Ls - j for j in sj))
+        done += 8 * d * (Ls * Lp + tri(Ls)) * G + 6 * d * col_pairs * G
+    desc = (f"oracle/ fp64 (C, OpenMP), Phase B fwd+bwd of {len(chosen)} (suffix, KV head) units "
+            f"[{chosen[0]}..{chosen[-1]}] x {G} q-heads: all suffix rows + every "
+            f"{'' if stride == 1 else str(stride) + '-th '}key column = "
+            f"{done / flops(shape)['step'] * 100:.2f}% of a step's algorithmic flops")
+    return dt, float(done), desc, oracle.max_threads()
+
+
+def run_reference(args, rank: int) -> None:
+    if rank != 0:
+        return
+    shape = pick_config(args.config)
+    times, work, desc, thr = [], 0.0, "", 0
+    # bound the whole run to ~1.2e12 algorithmic flops (a few minutes of host time)
+    budget = min(args.cpu_budget, 1.2e12 / max(1, args.warmup + args.steps))
+    for i in range(args.warmup + args.steps):
+        dt, work, desc, thr = oracle_sample(shape, budget)
+        if i >= args.warmup:
+            times.append(dt)
+    ms = 1e3 * sum(times) / len(times)
+    val = work / (ms * 1e-3) / 1e12
+    out = dict(metric=METRIC, value=val, unit=UNIT, n_gpus=args.gpus, steps=args.steps,
+               warmup=args.warmup, ms_per_step=ms, higher_is_better=True, scaling="weak",
+               vs_baseline=None, dtype="f64", data="synthetic", impl="reference",
+               config=workload_config(shape, args.config),
+               cpu_baseline=dict(value=val, unit=UNIT, cores=thr, kind="oracle", sample=desc),
+               e2e=dict(value=val, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
+               gpu_launches=0)
+    print(json.dumps(out))
+
+
+def workload_config(shape, name: str) -> dict:
+    Ls = shape.Ls
+    return dict(workload=f"BASELINE.json configs[{ {'tiny': 0, '7b': 1, 'ragged': 2, '32k': 4}.get(name, 3) }] "
+                         f"{shape.name}: {shape.n_q_heads}q/{shape.n_kv_heads}kv heads, d={shape.head_dim}, "
+                         f"prefix {shape.Lp}, N={shape.N} suffixes of "
+                         f"{Ls[0] if len(set(Ls)) == 1 else f'{min(Ls)}..{max(Ls)}'} tokens "
+                         f"({100 * shape.Lp / (shape.Lp + sum(Ls) / max(1, len(Ls))):.0f}% prefix)",
+                seed=shape.seed, dist="N(0,1)/sqrt(d) -> bf16", parallelism="1 group per GPU")
+
+
+# --------------------------------------------------------------------------------------------------
+# GPU leg
+# --------------------------------------------------------------------------------------------------
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="7b")
+    ap.add_argument("--replay-steps", type=int, default=-1, help="-1: max(3, steps // 4); 0: skip")
+    ap.add_argument("--cpu-budget", type=float, default=6e11, help="algorithmic flops of the oracle sample")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2606_01143_b200 import binding as pf          # raises if libprefixflow.so is missing
+    from paper_2606_01143_b200 import inputs, schedule
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback of the product path)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+
+    shape = pick_config(args.config)
+    # weak scaling over independent rollout groups: rank r draws its own group
+    if world > 1:
+        shape.seed += 100000 * rank
+    F = flops(shape)
+    peaks = measured_peaks()
+    ctx = pf.pf_create(local_rank)
+    inp = inputs.make_group(shape)
+    g = schedule.to_device(inp, dev)
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    def timed(fn, steps):
+        """K steps between two CUDA events on the launch stream; max over ranks; returns ms/step."""
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record(stream)
+        for _ in range(steps):
+            fn()
+        e1.record(stream)
+        barrier()
+        ms = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms = float(t.item())
+        return ms / steps
+
+    step = lambda: schedule.run_prefixflow_step(ctx, g, stream)
+    torch.cuda.reset_peak_memory_stats()
+    for _ in range(args.warmup):
+        step()
+    n0 = pf.pf_counter(ctx, "kernel_launches")
+    with ClockSampler(local_rank) as clk:
+        ms_step = timed(step, args.steps)
+    launches = pf.pf_counter(ctx, "kernel_launches") - n0
+    peak_hbm = torch.cuda.max_memory_allocated()
+
+    # ---- same K steps with the per-kernel event brackets of the C ABI: per-phase kernel time ----
+    pf.pf_set_option(ctx, "profile", 1)
+    for k in range(4):
+        pf.pf_profile_read(ctx, k)
+    ms_step_prof = timed(step, args.steps)
+    prof = {}
+    for k, name in enumerate(["A_fwd", "B_fwd", "B_bwd", "C_bwd"]):
+        n, ms = pf.pf_profile_read(ctx, k)
+        prof[name] = dict(launches=n, ms_total=ms, ms_per_launch=ms / n if n else None)
+    pf.pf_set_option(ctx, "profile", 0)
+    steps = args.steps
+    ph_ms = {k: (v["ms_total"] / steps) for k, v in prof.items()}
+    tf = lambda fl, ms: (fl / (ms * 1e-3) / 1e12) if ms and ms > 0 else None
+    phases = dict(
+        A_fwd=dict(ms=ph_ms["A_fwd"], tflops=tf(F["A"], ph_ms["A_fwd"])),
+        B_fwd=dict(ms=ph_ms["B_fwd"], tflops=tf(F["B_fwd"], ph_ms["B_fwd"])),
+        B_bwd=dict(ms=ph_ms["B_bwd"], tflops=tf(F["B_bwd"], ph_ms["B_bwd"])),
+        C_bwd=dict(ms=ph_ms["C_bwd"], tflops=tf(F["C"], ph_ms["C_bwd"])))
+    b_ms = ph_ms["B_fwd"] + ph_ms["B_bwd"]
+    phaseB_tflops = tf(F["B_fwd"] + F["B_bwd"], b_ms)
+    other_ms = ms_step_prof - sum(ph_ms.values())
+
+    # roofline of the dominant kernel: attn_bwd_kernel as launched by pf_phaseB_bwd
+    nB = prof["B_bwd"]["launches"]
+    ach = tf(F["B_bwd"] * steps / nB, prof["B_bwd"]["ms_per_launch"]) if nB else None
+    kname = f"attn_bwd_kernel<{shape.head_dim}>"
+    roofline = dict(bound="tensor", kernel=kname + " (pf_phaseB_bwd)", achieved=ach,
+                    peak=peaks["sustained"], unit="TFLOP/s",
+                    frac=(ach / peaks["sustained"]) if ach else None,
+                    peak_kind="bf16 sustained, " + peaks["source"],
+                    frac_of_burst=(ach / peaks["burst"]) if ach else None, peak_burst=peaks["burst"],
+                    frac_of_nominal=(ach / 2250.0) if ach else None,
+                    flops_per_launch=F["B_bwd"] / max(1, shape.N),
+                    ms_per_launch=prof["B_bwd"]["ms_per_launch"],
+                    traffic=ncu_traffic(kname, args.config))
+
+    # ---- N-times replay baseline: the same kernels on every concatenated [P || S(i)] ----
+    replay = None
+    rsteps = max(3, args.steps // 4) if args.replay_steps < 0 else args.replay_steps
+    if rsteps > 0:
+        r = schedule.make_replay(g)
+        rstep = lambda: schedule.run_replay_step(ctx, r, stream)
+        for _ in range(2):
+            rstep()
+        ms_replay = timed(rstep, rsteps)
+        replay = dict(ms_per_step=ms_replay, steps=rsteps, tflops=tf(F["replay"], ms_replay),
+                      speedup=ms_replay / ms_step, ideal_speedup_pair_model=F["ideal_speedup"])
+        del r
+        torch.cuda.empty_cache()
+
+    # ---- end to end: pinned host inputs -> device, step, results -> pinned host, every step ----
+    e2e = None
+    if not args.no_e2e:
+        ins = [g.Q1, g.K1, g.V1, g.dO1] + g.Q2 + g.K2 + g.V2 + g.dO2
+        outs = [g.O1, g.LSE1, g.dQ1, g.dK1, g.dV1, g.gK1, g.gV1] + g.O2 + g.LSE2 + g.dQ2 + g.dK2 + g.dV2
+        h_in = [torch.empty(t.shape, dtype=t.dtype, pin_memory=True).copy_(t) for t in ins]
+        h_out = [torch.empty(t.shape, dtype=t.dtype, pin_memory=True) for t in outs]
+        bi = sum(t.numel() * t.element_size() for t in ins)
+        bo = sum(t.numel() * t.element_size() for t in outs)
+
+        def e2e_step():
+            for h, t in zip(h_in, ins):
+                pf.pf_prefetch(ctx, h, t, stream)          # cudaMemcpyAsync H2D through the C ABI
+            schedule.run_prefixflow_step(ctx, g, stream)
+            for t, h in zip(outs, h_out):
+                pf.pf_offload(ctx, t, h, stream)           # cudaMemcpyAsync D2H through the C ABI
+
+        for _ in range(2):
+            e2e_step()
+        ms_e2e = timed(e2e_step, max(3, args.steps // 2))
+        e2e = dict(value=world * F["step"] / (ms_e2e * 1e-3) / 1e12, unit=UNIT, ms_per_step=ms_e2e,
+                   h2d_bytes_per_step=bi, d2h_bytes_per_step=bo,
+                   note="pinned host inputs copied in and all outputs copied out every step, one stream")
+        del h_in, h_out
+
+    # ---- CPU oracle on a bounded sample (rank 0, N = 1 only) ----
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        dt, work, desc, thr = oracle_sample(shape, args.cpu_budget)
+        cpu = dict(value=work / dt / 1e12, unit=UNIT, cores=thr, kind="oracle", sample=desc,
+                   seconds=dt)
+
+    value = world * F["step"] / (ms_step * 1e-3) / 1e12
+    ws_bytes = sum(t.numel() * t.element_size() for t in
+                   [g.Q1, g.K1, g.V1, g.dO1, g.O1, g.dQ1, g.dK1, g.dV1, g.gK1, g.gV1] +
+                   g.Q2 + g.K2 + g.V2 + g.dO2 + g.O2 + g.dQ2 + g.dK2 + g.dV2)
+    cfg = workload_config(shape, args.config)
+    cfg["l2"] = (f"no explicit flush: one step touches {ws_bytes / 2 ** 20:.0f} MiB of inputs+outputs "
+                 f"(> 126 MiB L2) before any tensor is reused" if ws_bytes > L2_BYTES else
+                 f"working set {ws_bytes / 2 ** 20:.0f} MiB fits L2 (parity-size config; not a bench line)")
+    out = dict(
+        metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
+        ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="bf16",
+        data="synthetic", config=cfg, clocks=clk.summary(), e2e=e2e, gpu_launches=launches,
+        roofline=roofline, cpu_baseline=cpu,
+        phases=phases, phaseB=dict(ms=b_ms, tflops=phaseB_tflops,
+                                   pct_of_bf16_burst=100 * phaseB_tflops / peaks["burst"] if phaseB_tflops else None,
+                                   pct_of_bf16_sustained=100 * phaseB_tflops / peaks["sustained"] if phaseB_tflops else None,
+                                   pct_of_bf16_nominal=100 * phaseB_tflops / 2250.0 if phaseB_tflops else None),
+        ms_per_step_profiled=ms_step_prof, non_attention_ms=other_ms,
+        replay=replay, flops=dict(A=F["A"], B_fwd=F["B_fwd"], B_bwd=F["B_bwd"], C=F["C"], step=F["step"],
+                                  replay=F["replay"]),
+        peak_hbm_bytes=peak_hbm, peaks=peaks)
+    pf.pf_destroy(ctx)
+    if rank == 0:
+        print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -84,8 +84,9 @@ pf_status pf_set_option(pf_ctx* ctx, const char* name, int64_t value);
  * counter name.  Host-side bookkeeping only. */
 int64_t pf_counter(const pf_ctx* ctx, const char* name);
 
-/* Profiling read-out (needs option "profile" = 1).  kind: 0 = attention forward kernel,
- * 1 = attention backward kernel.  Synchronises on the recorded events, adds up their durations,
+/* Profiling read-out (needs option "profile" = 1).  kind: the call that launched the attention
+ * kernel -- 0 = pf_phaseA_fwd, 1 = pf_phaseB_fwd, 2 = pf_phaseB_bwd, 3 = pf_phaseC_bwd (forward
+ * kernel for 0/1, backward kernel for 2/3).  Synchronises on the recorded events, adds up their durations,
  * writes the number of launches and the total milliseconds since the previous read of that kind,
  * and recycles the events. */
 pf_status pf_profile_read(pf_ctx* ctx, int32_t kind, int64_t* launches, double* total_ms);

@@ -192,7 +192,7 @@ pf_status set_attrs() {
 template <int D>
 pf_status launch_fwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const pf_tensor& V1,
                      int64_t Lp, const pf_tensor& K2, const pf_tensor& V2, const pf_tensor& O,
-                     float* LSE, int64_t lse_stride, int64_t Lq, cudaStream_t s) {
+                     float* LSE, int64_t lse_stride, int64_t Lq, int prof_kind, cudaStream_t s) {
     pf_ctx* ctx = g->ctx;
     const int Hq = g->desc.n_q_heads, Hkv = g->desc.n_kv_heads;
     CUtensorMap mQ, mK1, mV1, mK2, mV2;
@@ -223,7 +223,7 @@ pf_status launch_fwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const
     const int nItems = p.nRB * p.G;
     dim3 grid((nItems + 1) / 2, Hkv);
     {
-        ProfScope prof(ctx, 0, s);
+        ProfScope prof(ctx, prof_kind, s);
         pf::attn_fwd_kernel<D><<<grid, pf::FwdCfg<D>::THREADS, pf::FwdCfg<D>::SMEM, s>>>(
             mQ, mK1, mV1, mK2, mV2, p);
     }
@@ -248,7 +248,7 @@ pf_status launch_bwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const
                      int64_t Lp, const pf_tensor& K2, const pf_tensor& V2, const pf_tensor& O,
                      const float* LSE, int64_t lse_stride, const pf_tensor& dO, float* accK1,
                      float* accV1, float* accK2, float* accV2, const pf_tensor& dQ, int64_t Lq,
-                     cudaStream_t s) {
+                     int prof_kind, cudaStream_t s) {
     pf_ctx* ctx = g->ctx;
     const int Hq = g->desc.n_q_heads, Hkv = g->desc.n_kv_heads, G = Hq / Hkv;
     const WsLayout w = ws_layout(g->desc, Lq);
@@ -298,7 +298,7 @@ pf_status launch_bwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const
     p.sigma = g->sigma;
     const int64_t items = int64_t(p.nPT + p.nQT) * Hkv * p.parts;
     {
-        ProfScope prof(ctx, 1, s);
+        ProfScope prof(ctx, prof_kind, s);
         pf::attn_bwd_kernel<D><<<unsigned(items), pf::BwdCfg<D>::THREADS, pf::BwdCfg<D>::SMEM, s>>>(
             mQ, mdO, mK1, mV1, mK2, mV2, p);
     }
@@ -526,8 +526,8 @@ pf_status pf_phaseA_fwd(pf_group* grp, pf_tensor Q1, pf_tensor O1, float* LSE1, 
     if (Lp > 0) {
         cudaStream_t s = static_cast<cudaStream_t>(stream);
         pf_tensor none = {nullptr, 0, 0};
-        st = d == 64 ? launch_fwd<64>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, Lp, s)
-                     : launch_fwd<128>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, Lp, s);
+        st = d == 64 ? launch_fwd<64>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, Lp, 0, s)
+                     : launch_fwd<128>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, Lp, 0, s);
         if (st) return st;
     }
     grp->state = 1;
@@ -556,8 +556,8 @@ pf_status pf_phaseB_fwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens
         if (Ls == 0) continue;
         const pf_tensor q = tok_offset(Q2, t0), k = tok_offset(K2, t0), v = tok_offset(V2, t0),
                         o = tok_offset(O2, t0);
-        st = d == 64 ? launch_fwd<64>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, Ls, s)
-                     : launch_fwd<128>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, Ls, s);
+        st = d == 64 ? launch_fwd<64>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, Ls, 1, s)
+                     : launch_fwd<128>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, Ls, 1, s);
         if (st) return st;
     }
     return PF_OK;
@@ -602,12 +602,12 @@ pf_status pf_phaseB_bwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens
                         o = tok_offset(O2, t0), dout = tok_offset(dO2, t0), dq = tok_offset(dQ2, t0);
         if (d == 64) {
             st = launch_bwd<64>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, dout,
-                                grp->gK1, grp->gV1, ak, av, dq, Ls, s);
+                                grp->gK1, grp->gV1, ak, av, dq, Ls, 2, s);
             if (!st) st = launch_convert_kv<64>(grp, ak, tok_offset(dK2, t0), Ls, s);
             if (!st) st = launch_convert_kv<64>(grp, av, tok_offset(dV2, t0), Ls, s);
         } else {
             st = launch_bwd<128>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, dout,
-                                 grp->gK1, grp->gV1, ak, av, dq, Ls, s);
+                                 grp->gK1, grp->gV1, ak, av, dq, Ls, 2, s);
             if (!st) st = launch_convert_kv<128>(grp, ak, tok_offset(dK2, t0), Ls, s);
             if (!st) st = launch_convert_kv<128>(grp, av, tok_offset(dV2, t0), Ls, s);
         }
@@ -647,12 +647,12 @@ pf_status pf_phaseC_bwd(pf_group* grp, pf_tensor Q1, pf_tensor O1, const float* 
         pf_tensor none = {nullptr, 0, 0};
         if (d == 64) {
             st = launch_bwd<64>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, dO1, nullptr,
-                                nullptr, ak, av, dQ1, Lp, s);
+                                nullptr, ak, av, dQ1, Lp, 3, s);
             if (!st) st = launch_convert_kv<64>(grp, ak, dK1, Lp, s);
             if (!st) st = launch_convert_kv<64>(grp, av, dV1, Lp, s);
         } else {
             st = launch_bwd<128>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, dO1, nullptr,
-                                 nullptr, ak, av, dQ1, Lp, s);
+                                 nullptr, ak, av, dQ1, Lp, 3, s);
             if (!st) st = launch_convert_kv<128>(grp, ak, dK1, Lp, s);
             if (!st) st = launch_convert_kv<128>(grp, av, dV1, Lp, s);
         }
