@@ -243,6 +243,8 @@ def main() -> None:
     ap.add_argument("--cpu-budget", type=float, default=6e11, help="algorithmic flops of the oracle sample")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--wave", type=int, default=1,
+                    help="suffixes packed per Phase-B call (PAPER.md:158 suffix microbatch); 0 = all N")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -274,7 +276,8 @@ def main() -> None:
     peaks = measured_peaks()
     ctx = pf.pf_create(local_rank)
     inp = inputs.make_group(shape)
-    g = schedule.to_device(inp, dev)
+    wave = args.wave if args.wave > 0 else max(1, shape.N)
+    g = schedule.to_device(inp, dev, wave=wave)
     stream = torch.cuda.current_stream()
 
     def barrier():
@@ -341,7 +344,7 @@ def main() -> None:
                     peak_kind="bf16 sustained, " + peaks["source"],
                     frac_of_burst=(ach / peaks["burst"]) if ach else None, peak_burst=peaks["burst"],
                     frac_of_nominal=(ach / 2250.0) if ach else None,
-                    flops_per_launch=F["B_bwd"] / max(1, shape.N),
+                    flops_per_launch=F["B_bwd"] / max(1, nB // max(1, steps)) if nB else None,
                     ms_per_launch=prof["B_bwd"]["ms_per_launch"],
                     traffic=ncu_traffic(kname, args.config))
 
@@ -396,6 +399,7 @@ def main() -> None:
                    [g.Q1, g.K1, g.V1, g.dO1, g.O1, g.dQ1, g.dK1, g.dV1, g.gK1, g.gV1] +
                    g.Q2 + g.K2 + g.V2 + g.dO2 + g.O2 + g.dQ2 + g.dK2 + g.dV2)
     cfg = workload_config(shape, args.config)
+    cfg["wave"] = wave
     cfg["l2"] = (f"no explicit flush: one step touches {ws_bytes / 2 ** 20:.0f} MiB of inputs+outputs "
                  f"(> 126 MiB L2) before any tensor is reused" if ws_bytes > L2_BYTES else
                  f"working set {ws_bytes / 2 ** 20:.0f} MiB fits L2 (parity-size config; not a bench line)")

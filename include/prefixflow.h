@@ -71,9 +71,12 @@ pf_status pf_destroy(pf_ctx* ctx);
 /* Message of the last failing call on this context (valid until the next call). */
 const char* pf_last_error(const pf_ctx* ctx);
 /* Options (host-side, take effect at the next launch):
- *   "bwd_head_parts" : split the G query heads of a KV head over this many CTAs per key tile in
- *                      the backward (0 = heuristic).  1 = every key tile owned by one CTA
- *                      (gK1/gV1 += without contention), G = maximal parallelism, most atomics. */
+ *   "bwd_pairs_per_item" : backward work split.  A CTA owns one tile of 128 prefix keys of one KV
+ *                      head and this many (sequence, query head) pairs of the wave (0 = heuristic).
+ *                      All pairs in one CTA = that key tile's gK1/gV1 rows are added by one CTA
+ *                      (no contention); 1 = maximal parallelism, most reduce-add traffic.
+ *   "bwd_heads_per_item" : the same for the tiles of a suffix's own (causal) keys: query heads of
+ *                      the KV head per CTA (0 = heuristic). */
 pf_status pf_set_option(pf_ctx* ctx, const char* name, int64_t value);
 
 /*   "profile"        : 1 = bracket every attention kernel launch (not the elementwise helpers)

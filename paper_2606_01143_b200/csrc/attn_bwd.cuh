@@ -1,58 +1,87 @@
-// attn_bwd.cuh -- sm_100a attention backward, KV-stationary, two KV sources.
+// attn_bwd.cuh -- sm_100a attention backward, KV-stationary, two KV sources, packed suffix waves.
 //
-// For one KV tile of 128 keys (of KV head g) and a range of query heads of that group, loop over
-// the query tiles that see it and issue the five contractions of flash backward
-// (PAPER.md:194-198):
-//     S^T  = K Q^T                 dP^T = V dO^T
+// One CTA owns one KV tile of 128 keys (of KV head g) and a chunk of the (sequence, query head)
+// pairs that see it, and loops over their query sub-tiles of 64 rows.  Per (key tile, query
+// sub-tile) it issues the five contractions of flash backward:
+//     S^T  = K Q^T                 dP^T = V dO^T                       [128 keys x 64 queries]
 //     P^T  = exp(sigma S^T - LSE)  dS^T = P^T o (dP^T - delta)
-//     dV  += P^T dO                dK  += dS^T Q            dQ_tile = dS K
-// dV and dK stay in TMEM for the whole loop (summing the G query heads of the KV head and all
-// query tiles) and are added once into an fp32 accumulator [L, Hkv, d]: for prefix-source keys
-// that accumulator IS the persistent gK1 / gV1 of the training-time KV cache -
-// Phase B adds the coupling term, Phase C adds the own-prefix term on top of it.  dQ tiles are
-// added into an fp32 workspace [Lq, Hq, d] (several KV tiles contribute to one query tile).
+//     dV  += P^T dO                dK  += dS^T Q                       [128 keys x D]
+//     dQ^T = K^T dS^T                                                  [D x 64 queries]
+// dV and dK stay in TMEM for the whole loop (summing the query heads of the KV head, all query
+// tiles and, for prefix keys, all sequences of the wave) and are added ONCE into an fp32
+// accumulator [L, Hkv, d] by a TMA tensor reduce-add: for prefix-source keys that accumulator IS
+// the persistent gK1 / gV1 of the training-time KV cache - Phase B adds the
+// coupling term, Phase C adds the own-prefix term on top of it.  dQ^T tiles are staged in shared
+// memory and bulk-reduce-added (cp.reduce.async.bulk .add.f32) into an fp32 tile-layout workspace
+// (several KV tiles contribute to one query tile); dq_finish_kernel rounds it to bf16.
 //
-//   warps 0-3  compute (thread j <-> key row j <-> TMEM lane j; for dQ: lane = query row)
-//   warp  4    TMA producer (K, V once; Q, dO, LSE, delta tiles through a 2-stage ring)
-//   warp  5    tcgen05.mma issuer (one thread)
-// TMEM (512 columns): S^T/P^T [0,128) | dP^T / dQ [128,256) | dV [256,256+D) | dK [256+D,256+2D)
+// Software pipeline (one iteration = one query sub-tile; b = it & 1):
+//   tensor pipe :  S^T(it+1) dP^T(it+1) | wait P(it) | dQ^T(it) dV(it) dK(it) | S^T(it+2) ...
+//   compute WGs :  ............ P^T,dS^T(it) .........|........ P^T,dS^T(it+1) ...........
+//   reduce WG   :  ........................ dQ^T(it-1) -> smem -> bulk reduce-add ..........
+//
+//   warps 0-3   compute, query columns [0,32)   (thread j <-> key row j <-> TMEM lane j)
+//   warps 4-7   compute, query columns [32,64)
+//   warps 8-11  dQ^T read-out (TMEM lane = d index) and reduce-add
+//   warp  12    TMA producer (K, V once; Q, dO, LSE, delta sub-tiles through a 3-stage ring)
+//   warp  13    tcgen05.mma issuer (one thread)
+// TMEM (512 columns): S^T/P^T 2 x 64 | dP^T/dQ^T 2 x 64 | dV [256,256+D) | dK [256+D,256+2D)
 #pragma once
 #include <cuda.h>
 #include "sm100_ptx.cuh"
 
 namespace pf {
 
+constexpr int kMaxSeqs = 32;  // sequences per launch (the host splits longer waves)
+
+// Sequences of one launch: packed back to back along the token axis.
+struct SeqTable {
+    int n;
+    int cu[kMaxSeqs + 1];   // token offset of sequence s in the packed tensors
+    int pqs[kMaxSeqs + 1];  // prefix sums of ceil(Ls / 64): first global query sub-tile of s
+    int ckt[kMaxSeqs + 1];  // prefix sums of ceil(Ls / 128): first global causal key tile of s
+};
+
 struct BwdParams {
-    float* dQacc;                  // [Lq, Hq, D] fp32, contiguous
-    float* accK1; float* accV1;    // prefix-source accumulators [Lp, Hkv, D] fp32 (gK1 / gV1)
-    float* accK2; float* accV2;    // causal-source accumulators [Lq, Hkv, D] fp32
-    const float* lse2;             // [Hq, Lpad] LSE * log2(e); +inf beyond Lq
-    const float* delta;            // [Hq, Lpad] rowsum(dO o O); 0 beyond Lq
-    int64_t stat_stride;           // Lpad (multiple of 128)
-    int Lq, Lp;
+    float* dQacc;                  // [Hq][nQS][2][D][32] fp32 tiles (16-B chunks xor-swizzled by d&7)
+    const float* lse2;             // [Hq, stat_stride] LSE * log2(e) at padded positions; +inf in pads
+    const float* delta;            // [Hq, stat_stride] rowsum(dO o O); 0 in pads
+    int64_t stat_stride;
+    int Lp;
     int Hq, Hkv, G;
-    int nQT;                       // ceil(Lq / 128)
     int nPT;                       // ceil(Lp / 128)
-    int parts, hpp;                // head parts per KV head, heads per part
+    int nQS;                       // total query sub-tiles = seq.pqs[seq.n]
+    int chunksP, ppcP;             // prefix items: the n*G (seq, head) pairs in chunks of ppcP
+    int chunksC, ppcC;             // causal items: the G heads of the sequence in chunks of ppcC
+    int nItemsP;                   // nPT * Hkv * chunksP
     float scale_log2;              // sigma * log2(e)
     float sigma;
+    SeqTable seq;
 };
 
 template <int D>
 struct BwdCfg {
-    static constexpr int QS = 2;                       // Q/dO ring depth
-    static constexpr int TILE = 128 * D * 2;
-    static constexpr int SUB = 128 * 64 * 2;
+    static constexpr int QS = 3;                       // Q/dO ring depth
     static constexpr int NSUB = D / 64;
+    static constexpr int KSUB = 128 * 128;             // [128 keys][64 bf16] swizzle-128B sub-tile
+    static constexpr int QSUB = 64 * 128;              // [64 queries][64 bf16]
+    static constexpr int KTILE = NSUB * KSUB;
+    static constexpr int QTILE = NSUB * QSUB;
+    static constexpr int DSB = 128 * 128;              // dS^T [128 keys][64 queries] bf16
+    static constexpr int DQB = D * 128;                // dQ^T half [D][32 queries] fp32
     static constexpr int OFF_K = 0;
-    static constexpr int OFF_V = TILE;
-    static constexpr int OFF_Q = 2 * TILE;             // QS tiles
-    static constexpr int OFF_DO = OFF_Q + QS * TILE;   // QS tiles
-    static constexpr int OFF_DS = OFF_DO + QS * TILE;  // 128 x 128 bf16 = 32 KB
-    static constexpr int OFF_STAT = OFF_DS + 32768;    // QS x (lse2[128], delta[128]) fp32
-    static constexpr int OFF_BAR = OFF_STAT + QS * 1024;
-    static constexpr int SMEM = OFF_BAR + 128;
-    static constexpr int THREADS = 192;
+    static constexpr int OFF_V = KTILE;
+    static constexpr int OFF_Q = 2 * KTILE;            // QS tiles
+    static constexpr int OFF_DO = OFF_Q + QS * QTILE;  // QS tiles
+    static constexpr int OFF_DS = OFF_DO + QS * QTILE; // 2 buffers
+    static constexpr int OFF_DQ = OFF_DS + 2 * DSB;    // 2 staging buffers
+    static constexpr int OFF_STAT = OFF_DQ + 2 * DQB;  // QS x (lse2[64], delta[64]) fp32
+    static constexpr int OFF_BAR = OFF_STAT + QS * 512;
+    static constexpr int SMEM = OFF_BAR + 256;
+    static constexpr int OFF_EPI = OFF_Q;              // epilogue staging: 2 x (D/32) x 16 KB
+    static constexpr int THREADS = 448;
+    static_assert(OFF_EPI + 2 * (D / 32) * 16384 <= OFF_DQ, "epilogue staging overlaps dQ staging");
+    static_assert(SMEM <= 232448, "shared memory budget");
 };
 
 __device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_t bytes,
@@ -62,51 +91,113 @@ __device__ __forceinline__ void bulk_load_1d(void* dst, const void* src, uint32_
         ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(src)), "r"(bytes), "r"(smem_u32(bar))
         : "memory");
 }
+// shared -> global, element-wise fp32 add, tracked by the bulk async-group of the issuing thread
+__device__ __forceinline__ void bulk_reduce_add_f32(float* dst, const void* src, uint32_t bytes) {
+    asm volatile(
+        "cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f32 [%0], [%1], %2;"
+        ::"l"(reinterpret_cast<uint64_t>(dst)), "r"(smem_u32(src)), "r"(bytes)
+        : "memory");
+}
+
+// Walks the (pair, query sub-tile) iterations of one item; every warp role runs the same walk.
+struct BwdIter {
+    const BwdParams& p;
+    int pair, pair_hi, g, qs_lo;
+    int s, h, qs, nqs, tok0, qsg0;
+    __device__ BwdIter(const BwdParams& p_, int pair_lo, int pair_hi_, int g_, int qs_lo_)
+        : p(p_), pair(pair_lo), pair_hi(pair_hi_), g(g_), qs_lo(qs_lo_) {
+        load();
+    }
+    __device__ __forceinline__ void load() {
+        while (pair < pair_hi) {
+            s = pair / p.G;
+            h = g * p.G + pair % p.G;
+            tok0 = p.seq.cu[s];
+            qsg0 = p.seq.pqs[s];
+            nqs = p.seq.pqs[s + 1] - qsg0;
+            qs = qs_lo;
+            if (qs < nqs) return;
+            ++pair;
+        }
+    }
+    __device__ __forceinline__ bool valid() const { return pair < pair_hi; }
+    __device__ __forceinline__ void next() {
+        if (++qs >= nqs) {
+            ++pair;
+            load();
+        }
+    }
+};
 
 template <int D>
-__global__ void __launch_bounds__(192, 1)
+__global__ void __launch_bounds__(448, 1)
 attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmdO,
                 const __grid_constant__ CUtensorMap tmK1, const __grid_constant__ CUtensorMap tmV1,
                 const __grid_constant__ CUtensorMap tmK2, const __grid_constant__ CUtensorMap tmV2,
-                const BwdParams p) {
+                const __grid_constant__ CUtensorMap tmAK1, const __grid_constant__ CUtensorMap tmAV1,
+                const __grid_constant__ CUtensorMap tmAK2, const __grid_constant__ CUtensorMap tmAV2,
+                const __grid_constant__ BwdParams p) {
     using C = BwdCfg<D>;
     extern __shared__ __align__(1024) uint8_t smem[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::OFF_BAR);
     uint64_t* bar_KV = bars;            // K and V landed
-    uint64_t* bar_Qf = bars + 1;        // [QS] Q, dO, lse2, delta tile landed
-    uint64_t* bar_Qe = bars + 3;        // [QS] tile consumed
-    uint64_t* bar_S = bars + 5;         // S^T and dP^T ready
-    uint64_t* bar_P = bars + 6;         // P^T (TMEM) and dS^T (smem) ready
-    uint64_t* bar_dQ = bars + 7;        // dQ tile (and dV, dK so far) ready
-    uint64_t* bar_dQfree = bars + 8;    // dQ tile read out of TMEM
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 10);
+    uint64_t* bar_Qf = bars + 1;        // [QS] Q, dO, lse2, delta sub-tile landed
+    uint64_t* bar_Qe = bars + 4;        // [QS] sub-tile consumed by its last MMA
+    uint64_t* bar_S = bars + 7;         // [2] S^T and dP^T of buffer b complete
+    uint64_t* bar_P = bars + 9;         // [2] P^T (TMEM) and dS^T (smem) of buffer b written
+    uint64_t* bar_dQ = bars + 11;       // [2] dQ^T of buffer b complete
+    uint64_t* bar_dQfree = bars + 13;   // [2] dQ^T of buffer b read out of TMEM
+    uint64_t* bar_done = bars + 15;     // every MMA of the item complete
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 16);
 
     const int tid = threadIdx.x, warp = tid >> 5;
     if ((smem_u32(smem) & 1023u) != 0) __trap();
 
-    // ---- item decode: prefix-source items first (heaviest), then causal tiles 0, 1, ... ----
-    const int per_tile = p.Hkv * p.parts;
+    // ---- item decode: prefix-source items first (heaviest), then the causal key tiles ----
     int item = blockIdx.x;
-    const bool pre = item < p.nPT * per_tile;
-    if (!pre) item -= p.nPT * per_tile;
-    const int kt = item / per_tile;                         // KV tile within its source
-    const int g = (item % per_tile) / p.parts;
-    const int part = item % p.parts;
-    const int h_lo = g * p.G + part * p.hpp;
-    const int h_hi = min(g * p.G + p.G, h_lo + p.hpp);
-    const int qt_lo = pre ? 0 : kt;                         // first query tile that sees this tile
-    const int n_qt = p.nQT - qt_lo;
-    const int n_iter = max(0, (h_hi - h_lo)) * n_qt;
-    const int Lkv = pre ? p.Lp : p.Lq;
-    const int kv0 = kt * 128;
+    const bool pre = item < p.nItemsP;
+    int kt, g, pair_lo, pair_hi, qs_lo, kvrow0;
+    if (pre) {
+        const int per = p.Hkv * p.chunksP;
+        kt = item / per;
+        const int r = item % per;
+        g = r / p.chunksP;
+        pair_lo = (r % p.chunksP) * p.ppcP;
+        pair_hi = min(p.seq.n * p.G, pair_lo + p.ppcP);
+        qs_lo = 0;
+        kvrow0 = kt * 128;
+    } else {
+        item -= p.nItemsP;
+        const int per = p.Hkv * p.chunksC;
+        const int ktg = item / per;
+        const int r = item % per;
+        int s = 0;
+        while (s + 1 < p.seq.n && p.seq.ckt[s + 1] <= ktg) ++s;
+        kt = ktg - p.seq.ckt[s];
+        g = r / p.chunksC;
+        const int h_lo = (r % p.chunksC) * p.ppcC;
+        pair_lo = s * p.G + h_lo;
+        pair_hi = s * p.G + min(p.G, h_lo + p.ppcC);
+        qs_lo = 2 * kt;
+        kvrow0 = p.seq.cu[s] + kt * 128;
+    }
+    int n_iter = 0;
+    for (int pr = pair_lo; pr < pair_hi; ++pr) {
+        const int s = pr / p.G;
+        n_iter += max(0, p.seq.pqs[s + 1] - p.seq.pqs[s] - qs_lo);
+    }
 
     if (tid == 0) {
         mbar_init(bar_KV, 1);
         for (int s = 0; s < C::QS; ++s) { mbar_init(&bar_Qf[s], 1); mbar_init(&bar_Qe[s], 1); }
-        mbar_init(bar_S, 1); mbar_init(bar_P, 128); mbar_init(bar_dQ, 1); mbar_init(bar_dQfree, 128);
+        for (int b = 0; b < 2; ++b) {
+            mbar_init(&bar_S[b], 1); mbar_init(&bar_P[b], 256);
+            mbar_init(&bar_dQ[b], 1); mbar_init(&bar_dQfree[b], 128);
+        }
+        mbar_init(bar_done, 1);
         fence_mbar_init();
     }
-    if (warp == 4) {
+    if (warp == 12) {
         tmem_alloc(tmem_slot, 512);
         if (elect_one()) {
             tma_prefetch_desc(&tmQ); tma_prefetch_desc(&tmdO);
@@ -117,195 +208,215 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
-    constexpr uint32_t T_ST = 0, T_DP = 128, T_DV = 256, T_DK = 256 + D;
+    constexpr uint32_t T_S = 0, T_DP = 128, T_DV = 256, T_DK = 256 + D;
 
-    if (warp == 4) {
+    if (warp == 12) {
         // =============================== TMA producer ===============================
         if (elect_one() && n_iter > 0) {
-            mbar_arrive_expect_tx(bar_KV, 2 * C::TILE);
+            mbar_arrive_expect_tx(bar_KV, 2 * C::KTILE);
             for (int k = 0; k < C::NSUB; ++k) {
-                tma_load_3d(smem + C::OFF_K + k * C::SUB, pre ? &tmK1 : &tmK2, bar_KV, 64 * k, g, kv0);
-                tma_load_3d(smem + C::OFF_V + k * C::SUB, pre ? &tmV1 : &tmV2, bar_KV, 64 * k, g, kv0);
+                tma_load_3d(smem + C::OFF_K + k * C::KSUB, pre ? &tmK1 : &tmK2, bar_KV, 64 * k, g, kvrow0);
+                tma_load_3d(smem + C::OFF_V + k * C::KSUB, pre ? &tmV1 : &tmV2, bar_KV, 64 * k, g, kvrow0);
             }
-            int it = 0;
-            for (int h = h_lo; h < h_hi; ++h) {
-                for (int qt = qt_lo; qt < p.nQT; ++qt, ++it) {
-                    const int st = it % C::QS;
-                    const uint32_t ph = (it / C::QS) & 1;
-                    mbar_wait(&bar_Qe[st], ph ^ 1);
-                    mbar_arrive_expect_tx(&bar_Qf[st], 2 * C::TILE + 1024);
-                    for (int k = 0; k < C::NSUB; ++k) {
-                        tma_load_3d(smem + C::OFF_Q + st * C::TILE + k * C::SUB, &tmQ, &bar_Qf[st],
-                                    64 * k, h, qt * 128);
-                        tma_load_3d(smem + C::OFF_DO + st * C::TILE + k * C::SUB, &tmdO, &bar_Qf[st],
-                                    64 * k, h, qt * 128);
-                    }
-                    float* stat = reinterpret_cast<float*>(smem + C::OFF_STAT + st * 1024);
-                    bulk_load_1d(stat, p.lse2 + int64_t(h) * p.stat_stride + qt * 128, 512, &bar_Qf[st]);
-                    bulk_load_1d(stat + 128, p.delta + int64_t(h) * p.stat_stride + qt * 128, 512,
-                                 &bar_Qf[st]);
+            BwdIter iter(p, pair_lo, pair_hi, g, qs_lo);
+            for (int it = 0; iter.valid(); ++it, iter.next()) {
+                const int st = it % C::QS;
+                mbar_wait(&bar_Qe[st], ((it / C::QS) & 1) ^ 1);
+                mbar_arrive_expect_tx(&bar_Qf[st], 2 * C::QTILE + 512);
+                const int row = iter.tok0 + iter.qs * 64;
+                for (int k = 0; k < C::NSUB; ++k) {
+                    tma_load_3d(smem + C::OFF_Q + st * C::QTILE + k * C::QSUB, &tmQ, &bar_Qf[st],
+                                64 * k, iter.h, row);
+                    tma_load_3d(smem + C::OFF_DO + st * C::QTILE + k * C::QSUB, &tmdO, &bar_Qf[st],
+                                64 * k, iter.h, row);
                 }
+                float* stat = reinterpret_cast<float*>(smem + C::OFF_STAT + st * 512);
+                const int64_t pos = int64_t(iter.h) * p.stat_stride + int64_t(iter.qsg0 + iter.qs) * 64;
+                bulk_load_1d(stat, p.lse2 + pos, 256, &bar_Qf[st]);
+                bulk_load_1d(stat + 64, p.delta + pos, 256, &bar_Qf[st]);
             }
         }
-    } else if (warp == 5) {
+    } else if (warp == 13) {
         // =============================== MMA issuer ===============================
         if (elect_one() && n_iter > 0) {
-            constexpr uint32_t id_kk = make_idesc_bf16(128, 128, false, false);  // S^T, dP^T
-            constexpr uint32_t id_kmn = make_idesc_bf16(128, D, false, true);    // dV, dK
-            constexpr uint32_t id_mnmn = make_idesc_bf16(128, D, true, true);    // dQ
-            const uint32_t sK = smem_u32(smem + C::OFF_K), sV = smem_u32(smem + C::OFF_V),
-                           sdS = smem_u32(smem + C::OFF_DS);
+            constexpr uint32_t id_s = make_idesc_bf16(128, 64, false, false);   // S^T, dP^T
+            constexpr uint32_t id_dq = make_idesc_bf16(128, 64, true, true);    // dQ^T
+            constexpr uint32_t id_kv = make_idesc_bf16(128, D, false, true);    // dV, dK
+            const uint32_t sK = smem_u32(smem + C::OFF_K), sV = smem_u32(smem + C::OFF_V);
+            const uint64_t dK_k = make_smem_desc_sw128(sK, 16, 1024);                 // K-major
+            const uint64_t dV_k = make_smem_desc_sw128(sV, 16, 1024);
+            const uint64_t dK_mn = make_smem_desc_sw128(sK, D == 128 ? C::KSUB : 0, 1024);  // K^T
+            auto issue_SdP = [&](int it) {
+                const int st = it % C::QS, b = it & 1;
+                const uint64_t dQ_k = make_smem_desc_sw128(smem_u32(smem + C::OFF_Q + st * C::QTILE), 16, 1024);
+                const uint64_t ddO_k = make_smem_desc_sw128(smem_u32(smem + C::OFF_DO + st * C::QTILE), 16, 1024);
+                mbar_wait(&bar_Qf[st], (it / C::QS) & 1);
+                if (it >= 2) mbar_wait(&bar_dQfree[b], ((it >> 1) - 1) & 1);  // dP^T region held dQ^T
+                tc_fence_after();
+#pragma unroll
+                for (int kk = 0; kk < D / 16; ++kk)   // S^T = K Q^T
+                    mma_ss(tmem + T_S + b * 64, dK_k + (((kk >> 2) * C::KSUB + (kk & 3) * 32) >> 4),
+                           dQ_k + (((kk >> 2) * C::QSUB + (kk & 3) * 32) >> 4), id_s, kk > 0);
+#pragma unroll
+                for (int kk = 0; kk < D / 16; ++kk)   // dP^T = V dO^T
+                    mma_ss(tmem + T_DP + b * 64, dV_k + (((kk >> 2) * C::KSUB + (kk & 3) * 32) >> 4),
+                           ddO_k + (((kk >> 2) * C::QSUB + (kk & 3) * 32) >> 4), id_s, kk > 0);
+                mma_commit(&bar_S[b]);
+            };
             mbar_wait(bar_KV, 0);
+            issue_SdP(0);
             for (int it = 0; it < n_iter; ++it) {
-                const int st = it % C::QS;
-                const uint32_t ph = (it / C::QS) & 1;
-                const uint32_t sQ = smem_u32(smem + C::OFF_Q + st * C::TILE);
-                const uint32_t sdO = smem_u32(smem + C::OFF_DO + st * C::TILE);
-                mbar_wait(&bar_Qf[st], ph);
-                if (it > 0) mbar_wait(bar_dQfree, (it - 1) & 1);  // dP^T region still holds dQ
+                if (it + 1 < n_iter) issue_SdP(it + 1);
+                const int st = it % C::QS, b = it & 1;
+                const uint32_t sQ = smem_u32(smem + C::OFF_Q + st * C::QTILE);
+                const uint32_t sdO = smem_u32(smem + C::OFF_DO + st * C::QTILE);
+                const uint32_t sdS = smem_u32(smem + C::OFF_DS + b * C::DSB);
+                const uint64_t dQ_mn = make_smem_desc_sw128(sQ, C::QSUB, 1024);
+                const uint64_t ddO_mn = make_smem_desc_sw128(sdO, C::QSUB, 1024);
+                const uint64_t ddS_k = make_smem_desc_sw128(sdS, 16, 1024);
+                const uint64_t ddS_mn = make_smem_desc_sw128(sdS, C::DSB, 1024);
+                mbar_wait(&bar_P[b], (it >> 1) & 1);
                 tc_fence_after();
 #pragma unroll
-                for (int kk = 0; kk < D / 16; ++kk) {  // S^T = K Q^T
-                    const uint32_t off = (kk >> 2) * C::SUB + (kk & 3) * 32;
-                    mma_ss(tmem + T_ST, make_smem_desc_sw128(sK + off, 16, 1024),
-                           make_smem_desc_sw128(sQ + off, 16, 1024), id_kk, kk > 0);
-                }
+                for (int kk = 0; kk < 8; ++kk)  // dQ^T = K^T dS^T  (A = K read MN-major, B = dS^T MN-major)
+                    mma_ss(tmem + T_DP + b * 64, dK_mn + ((kk * 2048) >> 4), ddS_mn + ((kk * 2048) >> 4),
+                           id_dq, kk > 0);
+                mma_commit(&bar_dQ[b]);
 #pragma unroll
-                for (int kk = 0; kk < D / 16; ++kk) {  // dP^T = V dO^T
-                    const uint32_t off = (kk >> 2) * C::SUB + (kk & 3) * 32;
-                    mma_ss(tmem + T_DP, make_smem_desc_sw128(sV + off, 16, 1024),
-                           make_smem_desc_sw128(sdO + off, 16, 1024), id_kk, kk > 0);
-                }
-                mma_commit(bar_S);
-                mbar_wait(bar_P, it & 1);
-                tc_fence_after();
+                for (int kk = 0; kk < 4; ++kk)  // dV += P^T dO   (A from TMEM, B = dO MN-major)
+                    mma_ts(tmem + T_DV, tmem + T_S + b * 64 + (kk >> 1) * 32 + (kk & 1) * 8,
+                           ddO_mn + ((kk * 2048) >> 4), id_kv, (it > 0 || kk > 0) ? 1u : 0u);
 #pragma unroll
-                for (int kk = 0; kk < 8; ++kk)  // dV += P^T dO   (A from TMEM, B = dO MN-major)
-                    mma_ts(tmem + T_DV, tmem + T_ST + kk * 8,
-                           make_smem_desc_sw128(sdO + kk * 2048, C::SUB, 1024), id_kmn,
+                for (int kk = 0; kk < 4; ++kk)  // dK += dS^T Q  (A = dS^T K-major, B = Q MN-major)
+                    mma_ss(tmem + T_DK, ddS_k + ((kk * 32) >> 4), dQ_mn + ((kk * 2048) >> 4), id_kv,
                            (it > 0 || kk > 0) ? 1u : 0u);
-#pragma unroll
-                for (int kk = 0; kk < 8; ++kk) {  // dK += dS^T Q  (A = dS^T K-major, B = Q MN-major)
-                    const uint32_t off = (kk >> 2) * C::SUB + (kk & 3) * 32;
-                    mma_ss(tmem + T_DK, make_smem_desc_sw128(sdS + off, 16, 1024),
-                           make_smem_desc_sw128(sQ + kk * 2048, C::SUB, 1024), id_kmn,
-                           (it > 0 || kk > 0) ? 1u : 0u);
-                }
-#pragma unroll
-                for (int kk = 0; kk < 8; ++kk)  // dQ = dS K  (A = dS^T read MN-major, B = K MN-major)
-                    mma_ss(tmem + T_DP, make_smem_desc_sw128(sdS + kk * 2048, C::SUB, 1024),
-                           make_smem_desc_sw128(sK + kk * 2048, C::SUB, 1024), id_mnmn, kk > 0);
                 mma_commit(&bar_Qe[st]);
-                mma_commit(bar_dQ);
             }
+            mma_commit(bar_done);
         }
-    } else if (n_iter > 0) {
-        // =============================== compute warps ===============================
-        const int j = tid;                                   // key row in tile / query row for dQ
-        const uint32_t lane_off = uint32_t(warp * 32) << 16;
-        const int kj = kv0 + j;                              // key index within its source
-        uint8_t* sdS = smem + C::OFF_DS;
-        int it = 0;
-        for (int h = h_lo; h < h_hi; ++h) {
-            for (int qt = qt_lo; qt < p.nQT; ++qt, ++it) {
-                const int st = it % C::QS;
-                const float* s_lse = reinterpret_cast<const float*>(smem + C::OFF_STAT + st * 1024);
-                const float* s_dl = s_lse + 128;
-                mbar_wait(&bar_Qf[st], (it / C::QS) & 1);    // lse2 / delta tile visible
-                mbar_wait(bar_S, it & 1);
+    } else if (warp < 8) {
+        // =============================== compute warpgroups ===============================
+        if (n_iter > 0) {
+            const int w = warp >> 2;                             // query-column half
+            const int j = tid & 127;                             // key row in tile == TMEM lane
+            const uint32_t lane_off = uint32_t((warp & 3) * 32) << 16;
+            const int kj = kt * 128 + j;                         // key index within its sequence
+            BwdIter iter(p, pair_lo, pair_hi, g, qs_lo);
+            for (int it = 0; iter.valid(); ++it, iter.next()) {
+                const int st = it % C::QS, b = it & 1;
+                const float4* s_lse = reinterpret_cast<const float4*>(smem + C::OFF_STAT + st * 512) + w * 8;
+                const float4* s_dl = s_lse + 16;
+                uint8_t* dsrow = smem + C::OFF_DS + b * C::DSB + j * 128;
+                mbar_wait(&bar_Qf[st], (it / C::QS) & 1);        // lse2 / delta visible
+                mbar_wait(&bar_S[b], (it >> 1) & 1);
                 tc_fence_after();
-                // visible query columns t' of this tile for key kj: causal => t >= kj
-                const int t0 = qt * 128;
-                int first = 0;                               // first visible column
-                if (!pre) first = kj - t0;                   // may be <= 0 (all visible) or > 127
-                const bool key_ok = kj < Lkv;
+                uint32_t s[32], dp[32];
+                tmem_ld32(tmem + T_S + b * 64 + w * 32 + lane_off, s);
+                tmem_ld32(tmem + T_DP + b * 64 + w * 32 + lane_off, dp);
+                tmem_wait_ld();
+                // causal source: query t sees key kj iff t >= kj; only diagonal sub-tiles need it
+                const bool diag = !pre && iter.qs * 64 < kt * 128 + 128;
+                const int first = kj - (iter.qs * 64 + w * 32);  // local columns < first are masked
+                uint32_t pk[16], dsk[16];
 #pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    uint32_t s[32], dp[32];
-                    tmem_ld32(tmem + T_ST + c * 32 + lane_off, s);
-                    tmem_ld32(tmem + T_DP + c * 32 + lane_off, dp);
-                    tmem_wait_ld();
-                    uint32_t pk[16], dsk[16];
+                for (int q4 = 0; q4 < 8; ++q4) {
+                    const float4 l = s_lse[q4], dl = s_dl[q4];
+                    const float lv[4] = {l.x, l.y, l.z, l.w}, dv[4] = {dl.x, dl.y, dl.z, dl.w};
+                    float pv[4], dsv[4];
 #pragma unroll
-                    for (int q = 0; q < 32; q += 2) {
-                        const int col = c * 32 + q;
-                        float p0 = fast_exp2(fmaf(__uint_as_float(s[q]), p.scale_log2, -s_lse[col]));
-                        float p1 = fast_exp2(fmaf(__uint_as_float(s[q + 1]), p.scale_log2, -s_lse[col + 1]));
-                        if (!key_ok || col < first) p0 = 0.f;
-                        if (!key_ok || col + 1 < first) p1 = 0.f;
-                        const float d0 = p0 * (__uint_as_float(dp[q]) - s_dl[col]);
-                        const float d1 = p1 * (__uint_as_float(dp[q + 1]) - s_dl[col + 1]);
-                        pk[q >> 1] = pack_bf16(p0, p1);
-                        dsk[q >> 1] = pack_bf16(d0, d1);
+                    for (int e = 0; e < 4; ++e) {
+                        const int q = q4 * 4 + e;
+                        float pe = fast_exp2(fmaf(__uint_as_float(s[q]), p.scale_log2, -lv[e]));
+                        if (diag && q < first) pe = 0.f;
+                        pv[e] = pe;
+                        dsv[e] = pe * (__uint_as_float(dp[q]) - dv[e]);
                     }
-                    // P^T -> TMEM (bf16 pairs): columns [16c, 16c+16) of the S^T region
-                    tmem_st16(tmem + T_ST + c * 16 + lane_off, pk);
-                    // dS^T -> smem, K-major swizzle-128B tiles [128 keys][64 queries]
-                    uint8_t* row = sdS + (c >> 1) * C::SUB + j * 128;
-#pragma unroll
-                    for (int ch = 0; ch < 4; ++ch) {
-                        const int chunk = (c & 1) * 4 + ch;
-                        *reinterpret_cast<uint4*>(row + ((chunk ^ (j & 7)) << 4)) =
-                            make_uint4(dsk[ch * 4], dsk[ch * 4 + 1], dsk[ch * 4 + 2], dsk[ch * 4 + 3]);
-                    }
+                    pk[q4 * 2] = pack_bf16(pv[0], pv[1]);
+                    pk[q4 * 2 + 1] = pack_bf16(pv[2], pv[3]);
+                    dsk[q4 * 2] = pack_bf16(dsv[0], dsv[1]);
+                    dsk[q4 * 2 + 1] = pack_bf16(dsv[2], dsv[3]);
                 }
+                // P^T -> TMEM (bf16 pairs) over the first 16 columns of this half's S^T region
+                tmem_st16(tmem + T_S + b * 64 + w * 32 + lane_off, pk);
+                // dS^T -> smem, K-major swizzle-128B tile [128 keys][64 queries]
+#pragma unroll
+                for (int ch = 0; ch < 4; ++ch)
+                    *reinterpret_cast<uint4*>(dsrow + (((w * 4 + ch) ^ (j & 7)) << 4)) =
+                        make_uint4(dsk[ch * 4], dsk[ch * 4 + 1], dsk[ch * 4 + 2], dsk[ch * 4 + 3]);
                 tmem_wait_st();
                 fence_proxy_async_smem();
                 tc_fence_before();
-                mbar_arrive(bar_P);
-                // ---- dQ tile: lane = query row ----
-                mbar_wait(bar_dQ, it & 1);
-                tc_fence_after();
-                const int t = t0 + j;
-                float* dq = p.dQacc + (int64_t(t) * p.Hq + h) * D;
-#pragma unroll
-                for (int c = 0; c < D / 32; ++c) {
-                    uint32_t v[32];
-                    tmem_ld32(tmem + T_DP + c * 32 + lane_off, v);
-                    tmem_wait_ld();
-                    if (t < p.Lq) {
-#pragma unroll
-                        for (int q = 0; q < 32; q += 4)
-                            red_add_v4(dq + c * 32 + q, __uint_as_float(v[q]), __uint_as_float(v[q + 1]),
-                                       __uint_as_float(v[q + 2]), __uint_as_float(v[q + 3]));
-                    }
-                }
-                tc_fence_before();
-                mbar_arrive(bar_dQfree);
+                mbar_arrive(&bar_P[b]);
             }
-        }
-        // ---- epilogue: dV, dK rows of this KV tile -> fp32 accumulators ----
-        // (the last bar_dQ commit covers every MMA issued before it)
-        {
-            const bool ok = kj < Lkv;  // ragged last tile: loads stay warp-uniform, stores are predicated
-            float* av = (pre ? p.accV1 : p.accV2) + (int64_t(kj) * p.Hkv + g) * D;
-            float* ak = (pre ? p.accK1 : p.accK2) + (int64_t(kj) * p.Hkv + g) * D;
+            // ---- epilogue: WG 0 adds dV, WG 1 adds sigma dK into the fp32 accumulators ----
+            mbar_wait(bar_done, 0);
+            tc_fence_after();
+            const float mul = w == 0 ? 1.f : p.sigma;
+            uint8_t* stage = smem + C::OFF_EPI + w * (D / 32) * 16384 + j * 128;
 #pragma unroll 1
             for (int c = 0; c < D / 32; ++c) {
                 uint32_t v[32];
-                tmem_ld32(tmem + T_DV + c * 32 + lane_off, v);
+                tmem_ld32(tmem + (w == 0 ? T_DV : T_DK) + c * 32 + lane_off, v);
                 tmem_wait_ld();
-                if (ok) {
 #pragma unroll
-                    for (int q = 0; q < 32; q += 4)
-                        red_add_v4(av + c * 32 + q, __uint_as_float(v[q]), __uint_as_float(v[q + 1]),
-                                   __uint_as_float(v[q + 2]), __uint_as_float(v[q + 3]));
-                }
-                tmem_ld32(tmem + T_DK + c * 32 + lane_off, v);
-                tmem_wait_ld();
-                if (ok) {
+                for (int ch = 0; ch < 8; ++ch)
+                    *reinterpret_cast<float4*>(stage + c * 16384 + ((ch ^ (j & 7)) << 4)) =
+                        make_float4(__uint_as_float(v[ch * 4]) * mul, __uint_as_float(v[ch * 4 + 1]) * mul,
+                                    __uint_as_float(v[ch * 4 + 2]) * mul, __uint_as_float(v[ch * 4 + 3]) * mul);
+            }
+            fence_proxy_async_smem();
+            named_bar_sync(1 + w, 128);
+            if (j == 0) {
+                const CUtensorMap* m = w == 0 ? (pre ? &tmAV1 : &tmAV2) : (pre ? &tmAK1 : &tmAK2);
+                for (int c = 0; c < D / 32; ++c)
+                    tma_reduce_add_3d(m, smem + C::OFF_EPI + (w * (D / 32) + c) * 16384, 32 * c, g, kvrow0);
+                bulk_commit();
+                bulk_wait<0>();
+            }
+        }
+    } else if (warp < 12) {
+        // =============================== dQ^T read-out and reduce-add ===============================
+        if (n_iter > 0) {
+            const int dl = tid & 127;                            // d index == TMEM lane
+            const uint32_t lane_off = uint32_t((warp & 3) * 32) << 16;
+            BwdIter iter(p, pair_lo, pair_hi, g, qs_lo);
+            for (int it = 0; iter.valid(); ++it, iter.next()) {
+                const int b = it & 1;
+                float* dst = p.dQacc + (int64_t(iter.h) * p.nQS + iter.qsg0 + iter.qs) * (2 * D * 32);
+                mbar_wait(&bar_dQ[b], (it >> 1) & 1);
+                tc_fence_after();
 #pragma unroll
-                    for (int q = 0; q < 32; q += 4)
-                        red_add_v4(ak + c * 32 + q, __uint_as_float(v[q]) * p.sigma,
-                                   __uint_as_float(v[q + 1]) * p.sigma, __uint_as_float(v[q + 2]) * p.sigma,
-                                   __uint_as_float(v[q + 3]) * p.sigma);
+                for (int half = 0; half < 2; ++half) {
+                    uint32_t v[32];
+                    tmem_ld32(tmem + T_DP + b * 64 + half * 32 + lane_off, v);
+                    tmem_wait_ld();
+                    if (half == 1) {
+                        tc_fence_before();
+                        mbar_arrive(&bar_dQfree[b]);
+                    }
+                    uint8_t* stage = smem + C::OFF_DQ + half * C::DQB;
+                    if (dl == 0) bulk_wait_read<1>();            // this buffer's previous reduce has read it
+                    named_bar_sync(3, 128);
+                    if (dl < D) {
+#pragma unroll
+                        for (int ch = 0; ch < 8; ++ch)
+                            *reinterpret_cast<uint4*>(stage + dl * 128 + ((ch ^ (dl & 7)) << 4)) =
+                                make_uint4(v[ch * 4], v[ch * 4 + 1], v[ch * 4 + 2], v[ch * 4 + 3]);
+                    }
+                    fence_proxy_async_smem();
+                    named_bar_sync(4, 128);
+                    if (dl == 0) {
+                        bulk_reduce_add_f32(dst + half * (D * 32), stage, C::DQB);
+                        bulk_commit();
+                    }
                 }
             }
+            if (dl == 0) bulk_wait<0>();
         }
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 4) tmem_dealloc(tmem, 512);
+    if (warp == 12) tmem_dealloc(tmem, 512);
 }
 
 }  // namespace pf

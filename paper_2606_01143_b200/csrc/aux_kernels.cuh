@@ -1,12 +1,14 @@
 // aux_kernels.cuh -- HBM-bound helpers around the attention backward (all elementwise / row-wise):
 //   bwd_preprocess : delta[h,t] = <dO[t,h], O[t,h]>,  lse2 = LSE * log2(e),
-//                    both padded to a multiple of 128 rows (+inf / 0) for the tile loads
+//                    every sequence padded to a multiple of 64 rows (+inf / 0) for the tile loads
+//   dq_finish      : fp32 dQ^T tile workspace of the backward -> bf16 dQ rows
 //   acc_to_bf16    : fp32 staging [L,H,D] (contiguous) * scale -> bf16 strided output
 // Each thread moves 16 bytes of bf16 (8 elements); rows are coalesced along d.
 #pragma once
 #include <cuda_runtime.h>
 #include <cuda_bf16.h>
 #include <stdint.h>
+#include "attn_bwd.cuh"  // SeqTable
 
 namespace pf {
 
@@ -14,21 +16,29 @@ __device__ __forceinline__ float2 bf2_to_f2(uint32_t u) {
     return make_float2(__uint_as_float(u << 16), __uint_as_float(u & 0xffff0000u));
 }
 
-// grid: (ceil(Lpad * D/8 / 256), Hq); one row (t,h) is handled by D/8 consecutive threads
+// grid: (ceil(nQS*64 * D/8 / 256), Hq); one padded position is handled by D/8 consecutive threads.
+// Padded positions: sequence s of the launch owns positions [64*pqs[s], 64*pqs[s+1]).
 template <int D>
 __global__ void __launch_bounds__(256)
 bwd_preprocess_kernel(const __nv_bfloat16* __restrict__ O, int64_t o_st, int64_t o_sh,
                       const __nv_bfloat16* __restrict__ dO, int64_t do_st, int64_t do_sh,
                       const float* __restrict__ LSE, int64_t lse_stride, float* __restrict__ lse2,
-                      float* __restrict__ delta, int64_t stat_stride, int Lq, int Lpad) {
+                      float* __restrict__ delta, int64_t stat_stride,
+                      const __grid_constant__ SeqTable seq) {
     constexpr int TPR = D / 8;  // threads per row
     const int h = blockIdx.y;
     const int64_t gid = int64_t(blockIdx.x) * 256 + threadIdx.x;
-    const int t = int(gid / TPR), c = int(gid % TPR);
+    const int pp = int(gid / TPR), c = int(gid % TPR);
+    const int npad = seq.pqs[seq.n] * 64;
+    int s = 0;
+    while (s + 1 < seq.n && seq.pqs[s + 1] * 64 <= pp) ++s;
+    const int tl = pp - seq.pqs[s] * 64;                       // row within its sequence
+    const bool ok = pp < npad && tl < seq.cu[s + 1] - seq.cu[s];
+    const int64_t t = seq.cu[s] + tl;                          // packed token row
     float acc = 0.f;
-    if (t < Lq) {
-        const uint4 a = *reinterpret_cast<const uint4*>(O + int64_t(t) * o_st + int64_t(h) * o_sh + c * 8);
-        const uint4 b = *reinterpret_cast<const uint4*>(dO + int64_t(t) * do_st + int64_t(h) * do_sh + c * 8);
+    if (ok) {
+        const uint4 a = *reinterpret_cast<const uint4*>(O + t * o_st + int64_t(h) * o_sh + c * 8);
+        const uint4 b = *reinterpret_cast<const uint4*>(dO + t * do_st + int64_t(h) * do_sh + c * 8);
         const uint32_t aw[4] = {a.x, a.y, a.z, a.w}, bw[4] = {b.x, b.y, b.z, b.w};
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
@@ -39,11 +49,48 @@ bwd_preprocess_kernel(const __nv_bfloat16* __restrict__ O, int64_t o_st, int64_t
     }
 #pragma unroll
     for (int o = TPR / 2; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    if (c == 0 && t < Lpad) {
-        const bool ok = t < Lq;
-        delta[int64_t(h) * stat_stride + t] = ok ? acc : 0.f;
-        lse2[int64_t(h) * stat_stride + t] =
+    if (c == 0 && pp < npad) {
+        delta[int64_t(h) * stat_stride + pp] = ok ? acc : 0.f;
+        lse2[int64_t(h) * stat_stride + pp] =
             ok ? LSE[int64_t(h) * lse_stride + t] * 1.4426950408889634f : __int_as_float(0x7f800000);
+    }
+}
+
+// dQ^T tiles of the backward (fp32, [Hq][nQS][2][D][32], 16-byte chunks of each 128-byte row
+// xor-swizzled by d & 7) -> dQ bf16 [t, h, :] = bf16_rne(sigma * dQ).  grid (nQS, Hq), 256 threads.
+template <int D>
+__global__ void __launch_bounds__(256)
+dq_finish_kernel(const float* __restrict__ acc, __nv_bfloat16* __restrict__ dst, int64_t d_st,
+                 int64_t d_sh, float scale, const __grid_constant__ SeqTable seq) {
+    __shared__ float tile[64][D + 1];
+    const int qsg = blockIdx.x, h = blockIdx.y;
+    const int nQS = seq.pqs[seq.n];
+    int s = 0;
+    while (s + 1 < seq.n && seq.pqs[s + 1] <= qsg) ++s;
+    const int t0 = (qsg - seq.pqs[s]) * 64;                    // first row of the tile in its sequence
+    const int Ls = seq.cu[s + 1] - seq.cu[s];
+    const float4* src = reinterpret_cast<const float4*>(acc + (int64_t(h) * nQS + qsg) * (2 * D * 32));
+    for (int i = threadIdx.x; i < 2 * D * 8; i += 256) {      // i = (half * D + d) * 8 + physical chunk
+        const float4 v = src[i];
+        const int pc = i & 7, d = (i >> 3) % D, half = (i >> 3) / D;
+        const int q = half * 32 + ((pc ^ (d & 7)) << 2);
+        tile[q][d] = v.x; tile[q + 1][d] = v.y; tile[q + 2][d] = v.z; tile[q + 3][d] = v.w;
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < 64 * (D / 8); i += 256) {
+        const int q = i / (D / 8), c = i % (D / 8);
+        if (t0 + q >= Ls) continue;
+        const float* r = &tile[q][c * 8];
+        __nv_bfloat162 p0 = __floats2bfloat162_rn(r[0] * scale, r[1] * scale);
+        __nv_bfloat162 p1 = __floats2bfloat162_rn(r[2] * scale, r[3] * scale);
+        __nv_bfloat162 p2 = __floats2bfloat162_rn(r[4] * scale, r[5] * scale);
+        __nv_bfloat162 p3 = __floats2bfloat162_rn(r[6] * scale, r[7] * scale);
+        uint4 v;
+        v.x = *reinterpret_cast<uint32_t*>(&p0);
+        v.y = *reinterpret_cast<uint32_t*>(&p1);
+        v.z = *reinterpret_cast<uint32_t*>(&p2);
+        v.w = *reinterpret_cast<uint32_t*>(&p3);
+        *reinterpret_cast<uint4*>(dst + (int64_t(seq.cu[s]) + t0 + q) * d_st + int64_t(h) * d_sh + c * 8) = v;
     }
 }
 

@@ -36,7 +36,8 @@ struct pf_ctx {
     int device = 0;
     int num_sms = 0;
     EncodeTiledFn encode = nullptr;
-    int bwd_head_parts = 0;  // 0 = heuristic
+    int bwd_pairs_per_item = 0;  // (seq, head) pairs per prefix-tile CTA; 0 = heuristic
+    int bwd_heads_per_item = 0;  // query heads per causal-tile CTA; 0 = heuristic
     bool profile = false;
     int64_t n_launches = 0;
     std::vector<ProfRec> prof;         // recorded, not yet read
@@ -54,6 +55,7 @@ struct pf_group {
     float* gV1;
     uint8_t* ws;
     size_t ws_bytes;
+    int64_t ws_cap;  // padded token positions the workspace holds (multiple of 64)
     int state;  // 0 begun, 1 A done, 2 C done
 };
 
@@ -136,10 +138,10 @@ pf_status check_tensor(pf_ctx* ctx, const char* name, const pf_tensor& t, int64_
     return PF_OK;
 }
 
-// 3-D map {d, H, L}, box {64, 1, 128}, swizzle-128B: one load = a [128 tokens][64 elements]
+// 3-D map {d, H, L}, box {64, 1, rows}, swizzle-128B: one load = a [rows tokens][64 elements]
 // K-major sub-tile of one head; rows past L are zero-filled.
 pf_status make_map(pf_ctx* ctx, CUtensorMap* m, const char* name, const pf_tensor& t, int64_t L,
-                   int H, int d) {
+                   int H, int d, int rows = 128) {
     if (L == 0) {
         memset(m, 0, sizeof(*m));
         return PF_OK;
@@ -147,7 +149,7 @@ pf_status make_map(pf_ctx* ctx, CUtensorMap* m, const char* name, const pf_tenso
     cuuint64_t dims[3] = {cuuint64_t(d), cuuint64_t(H), cuuint64_t(L)};
     cuuint64_t strides[2] = {cuuint64_t((H > 1 ? t.stride_head : int64_t(d)) * 2),
                              cuuint64_t(t.stride_tok * 2)};
-    cuuint32_t box[3] = {64, 1, 128};
+    cuuint32_t box[3] = {64, 1, cuuint32_t(rows)};
     cuuint32_t es[3] = {1, 1, 1};
     CUresult r = ctx->encode(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, t.ptr, dims, strides, box, es,
                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
@@ -158,22 +160,57 @@ pf_status make_map(pf_ctx* ctx, CUtensorMap* m, const char* name, const pf_tenso
     return PF_OK;
 }
 
+// fp32 accumulator [L, H, d] contiguous: box {32, 1, 128} (128-byte rows, swizzle-128B) for the
+// reduce-add of a [128 keys][32 floats] staging tile; rows past L are clipped.
+pf_status make_acc_map(pf_ctx* ctx, CUtensorMap* m, const char* name, float* ptr, int64_t L, int H,
+                       int d) {
+    if (L == 0 || !ptr) {
+        memset(m, 0, sizeof(*m));
+        return PF_OK;
+    }
+    cuuint64_t dims[3] = {cuuint64_t(d), cuuint64_t(H), cuuint64_t(L)};
+    cuuint64_t strides[2] = {cuuint64_t(d) * 4, cuuint64_t(H) * d * 4};
+    cuuint32_t box[3] = {32, 1, 128};
+    cuuint32_t es[3] = {1, 1, 1};
+    CUresult r = ctx->encode(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, ptr, dims, strides, box, es,
+                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                             CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS)
+        return fail(ctx, PF_CUDA_ERROR, "cuTensorMapEncodeTiled(%s) failed with CUresult %d", name,
+                    int(r));
+    return PF_OK;
+}
+
+// Workspace carving for `cap` padded token positions (multiple of 64): softmax statistics, the
+// fp32 dQ^T tiles and the fp32 dK2/dV2 staging of the causal source.
 struct WsLayout {
     int64_t off_lse2, off_delta, off_dq, off_ak, off_av, total;
     int64_t stat_stride;
 };
 
-WsLayout ws_layout(const pf_desc& d, int64_t Lmax) {
+int64_t ws_bytes_per_pos(const pf_desc& d) {
+    return int64_t(d.n_q_heads) * 8 + int64_t(d.n_q_heads) * d.head_dim * 4 +
+           int64_t(d.n_kv_heads) * d.head_dim * 8;
+}
+
+WsLayout ws_layout(const pf_desc& d, int64_t cap) {
     WsLayout w;
-    w.stat_stride = align_up(Lmax, 128);
+    w.stat_stride = cap;
     int64_t o = 0;
-    w.off_lse2 = o; o += align_up(int64_t(d.n_q_heads) * w.stat_stride * 4, kAlign);
-    w.off_delta = o; o += align_up(int64_t(d.n_q_heads) * w.stat_stride * 4, kAlign);
-    w.off_dq = o; o += align_up(Lmax * d.n_q_heads * d.head_dim * 4, kAlign);
-    w.off_ak = o; o += align_up(Lmax * d.n_kv_heads * d.head_dim * 4, kAlign);
-    w.off_av = o; o += align_up(Lmax * d.n_kv_heads * d.head_dim * 4, kAlign);
+    w.off_lse2 = o; o += align_up(int64_t(d.n_q_heads) * cap * 4, kAlign);
+    w.off_delta = o; o += align_up(int64_t(d.n_q_heads) * cap * 4, kAlign);
+    w.off_dq = o; o += align_up(cap * d.n_q_heads * d.head_dim * 4, kAlign);
+    w.off_ak = o; o += align_up(cap * d.n_kv_heads * d.head_dim * 4, kAlign);
+    w.off_av = o; o += align_up(cap * d.n_kv_heads * d.head_dim * 4, kAlign);
     w.total = o;
     return w;
+}
+
+// largest capacity whose layout fits `bytes`
+int64_t ws_capacity(const pf_desc& d, size_t bytes) {
+    const int64_t slack = 6 * kAlign;
+    if (int64_t(bytes) <= slack) return 0;
+    return (int64_t(bytes) - slack) / ws_bytes_per_pos(d) / 64 * 64;
 }
 
 template <int D>
@@ -232,83 +269,111 @@ pf_status launch_fwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const
     return PF_OK;
 }
 
-int pick_parts(const pf_ctx* ctx, int G, int64_t n_tiles_times_hkv) {
-    if (ctx->bwd_head_parts > 0) return ctx->bwd_head_parts < G ? ctx->bwd_head_parts : G;
-    // heuristic: at least ~3 CTAs per SM of work items, but never more parts than heads
-    int parts = 1;
-    while (parts < G && n_tiles_times_hkv * parts < 3 * int64_t(ctx->num_sms)) ++parts;
-    return parts;
+// Sequence table of one backward launch from host offsets cu[0..n] (cu[0] = 0, n <= kMaxSeqs)
+pf::SeqTable make_seq_table(int n, const int64_t* cu) {
+    pf::SeqTable t;
+    memset(&t, 0, sizeof(t));
+    t.n = n;
+    for (int s = 0; s <= n; ++s) t.cu[s] = int(cu[s]);
+    for (int s = 0; s < n; ++s) {
+        const int Ls = t.cu[s + 1] - t.cu[s];
+        t.pqs[s + 1] = t.pqs[s] + (Ls + 63) / 64;
+        t.ckt[s + 1] = t.ckt[s] + (Ls + 127) / 128;
+    }
+    return t;
 }
 
-// ---- backward launch.  Keys of the prefix source accumulate into accK1/accV1 (fp32, +=),
-// keys of the causal source into accK2/accV2 (fp32, +=); dQ goes through the fp32 staging buffer
-// and is rounded to bf16 once all key tiles have contributed.
+// ---- backward launch over a wave of n sequences packed along the token axis.  Keys of the prefix
+// source accumulate into accK1/accV1 (fp32, +=), keys of the causal source into accK2/accV2
+// (fp32 [total, Hkv, d], +=); dQ goes through the fp32 tile workspace and is rounded to bf16 once
+// all key tiles have contributed.
 template <int D>
 pf_status launch_bwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const pf_tensor& V1,
                      int64_t Lp, const pf_tensor& K2, const pf_tensor& V2, const pf_tensor& O,
                      const float* LSE, int64_t lse_stride, const pf_tensor& dO, float* accK1,
-                     float* accV1, float* accK2, float* accV2, const pf_tensor& dQ, int64_t Lq,
-                     int prof_kind, cudaStream_t s) {
+                     float* accV1, float* accK2, float* accV2, const pf_tensor& dQ, int n,
+                     const int64_t* cu, int prof_kind, cudaStream_t s) {
     pf_ctx* ctx = g->ctx;
     const int Hq = g->desc.n_q_heads, Hkv = g->desc.n_kv_heads, G = Hq / Hkv;
-    const WsLayout w = ws_layout(g->desc, Lq);
-    if (size_t(w.total) > g->ws_bytes)
-        return fail(ctx, PF_WORKSPACE, "workspace too small: need %lld bytes for %lld tokens, have %zu",
-                    (long long)w.total, (long long)Lq, g->ws_bytes);
+    const pf::SeqTable seq = make_seq_table(n, cu);
+    const int64_t total = cu[n];
+    const int nQS = seq.pqs[n];
+    const int64_t npad = int64_t(nQS) * 64;
+    if (npad > g->ws_cap)
+        return fail(ctx, PF_WORKSPACE, "workspace too small: %lld padded positions, capacity %lld",
+                    (long long)npad, (long long)g->ws_cap);
+    const WsLayout w = ws_layout(g->desc, g->ws_cap);
     float* lse2 = reinterpret_cast<float*>(g->ws + w.off_lse2);
     float* delta = reinterpret_cast<float*>(g->ws + w.off_delta);
     float* dqacc = reinterpret_cast<float*>(g->ws + w.off_dq);
-    const int Lpad = int(w.stat_stride);
 
-    CUtensorMap mQ, mdO, mK1, mV1, mK2, mV2;
+    CUtensorMap mQ, mdO, mK1, mV1, mK2, mV2, mAK1, mAV1, mAK2, mAV2;
     pf_status st;
-    if ((st = make_map(ctx, &mQ, "Q", Q, Lq, Hq, D))) return st;
-    if ((st = make_map(ctx, &mdO, "dO", dO, Lq, Hq, D))) return st;
-    if ((st = make_map(ctx, &mK2, "K", K2, Lq, Hkv, D))) return st;
-    if ((st = make_map(ctx, &mV2, "V", V2, Lq, Hkv, D))) return st;
+    if ((st = make_map(ctx, &mQ, "Q", Q, total, Hq, D, 64))) return st;
+    if ((st = make_map(ctx, &mdO, "dO", dO, total, Hq, D, 64))) return st;
+    if ((st = make_map(ctx, &mK2, "K", K2, total, Hkv, D))) return st;
+    if ((st = make_map(ctx, &mV2, "V", V2, total, Hkv, D))) return st;
+    if ((st = make_acc_map(ctx, &mAK2, "accK2", accK2, total, Hkv, D))) return st;
+    if ((st = make_acc_map(ctx, &mAV2, "accV2", accV2, total, Hkv, D))) return st;
     if (Lp > 0) {
         if ((st = make_map(ctx, &mK1, "K1", K1, Lp, Hkv, D))) return st;
         if ((st = make_map(ctx, &mV1, "V1", V1, Lp, Hkv, D))) return st;
+        if ((st = make_acc_map(ctx, &mAK1, "gK1", accK1, Lp, Hkv, D))) return st;
+        if ((st = make_acc_map(ctx, &mAV1, "gV1", accV1, Lp, Hkv, D))) return st;
     } else {
-        mK1 = mK2;
-        mV1 = mV2;
+        mK1 = mK2; mV1 = mV2; mAK1 = mAK2; mAV1 = mAV2;
     }
-    PF_CUDA(ctx, cudaMemsetAsync(dqacc, 0, size_t(Lq) * Hq * D * 4, s));
+    PF_CUDA(ctx, cudaMemsetAsync(dqacc, 0, size_t(npad) * Hq * D * 4, s));
     {
-        const int64_t threads = int64_t(Lpad) * (D / 8);
+        const int64_t threads = npad * (D / 8);
         dim3 grid(unsigned((threads + 255) / 256), Hq);
         pf::bwd_preprocess_kernel<D><<<grid, 256, 0, s>>>(
             static_cast<const __nv_bfloat16*>(O.ptr), O.stride_tok, O.stride_head,
             static_cast<const __nv_bfloat16*>(dO.ptr), dO.stride_tok, dO.stride_head, LSE, lse_stride,
-            lse2, delta, w.stat_stride, int(Lq), Lpad);
+            lse2, delta, w.stat_stride, seq);
         PF_CUDA(ctx, cudaGetLastError());
         ctx->n_launches += 1;
     }
     pf::BwdParams p;
     p.dQacc = dqacc;
-    p.accK1 = accK1; p.accV1 = accV1; p.accK2 = accK2; p.accV2 = accV2;
     p.lse2 = lse2; p.delta = delta; p.stat_stride = w.stat_stride;
-    p.Lq = int(Lq); p.Lp = int(Lp);
+    p.Lp = int(Lp);
     p.Hq = Hq; p.Hkv = Hkv; p.G = G;
-    p.nQT = int((Lq + 127) / 128);
     p.nPT = int((Lp + 127) / 128);
-    p.parts = pick_parts(ctx, G, int64_t(p.nQT + p.nPT) * Hkv);
-    p.hpp = (G + p.parts - 1) / p.parts;
+    p.nQS = nQS;
+    p.seq = seq;
+    // ---- item sizing: aim at >= ~6 items per SM, each long enough to amortise its prologue
+    // (K/V load, TMEM allocation) and epilogue (dK/dV reduce-add)
+    int64_t iters = int64_t(p.nPT) * Hkv * G * nQS;
+    for (int i = 0; i < n; ++i) {
+        const int nqs = seq.pqs[i + 1] - seq.pqs[i], nkt = seq.ckt[i + 1] - seq.ckt[i];
+        for (int kt = 0; kt < nkt; ++kt) iters += int64_t(Hkv) * G * (nqs - 2 * kt > 0 ? nqs - 2 * kt : 0);
+    }
+    const double target = std::fmin(192.0, std::fmax(24.0, double(iters) / (6.0 * ctx->num_sms)));
+    const double avg_nqs = n > 0 ? double(nQS) / n : 1.0;
+    const int pairs = n * G;
+    int ppcP = ctx->bwd_pairs_per_item > 0 ? ctx->bwd_pairs_per_item
+                                           : int(std::lround(target / std::fmax(1.0, avg_nqs)));
+    ppcP = ppcP < 1 ? 1 : (ppcP > pairs ? pairs : ppcP);
+    int ppcC = ctx->bwd_heads_per_item > 0 ? ctx->bwd_heads_per_item
+                                           : int(std::lround(target / std::fmax(1.0, avg_nqs / 2)));
+    ppcC = ppcC < 1 ? 1 : (ppcC > G ? G : ppcC);
+    p.ppcP = ppcP; p.chunksP = (pairs + ppcP - 1) / ppcP;
+    p.ppcC = ppcC; p.chunksC = (G + ppcC - 1) / ppcC;
+    p.nItemsP = p.nPT * Hkv * p.chunksP;
     p.scale_log2 = g->sigma * 1.4426950408889634f;
     p.sigma = g->sigma;
-    const int64_t items = int64_t(p.nPT + p.nQT) * Hkv * p.parts;
-    {
+    const int64_t items = int64_t(p.nItemsP) + int64_t(seq.ckt[n]) * Hkv * p.chunksC;
+    if (items > 0) {
         ProfScope prof(ctx, prof_kind, s);
         pf::attn_bwd_kernel<D><<<unsigned(items), pf::BwdCfg<D>::THREADS, pf::BwdCfg<D>::SMEM, s>>>(
-            mQ, mdO, mK1, mV1, mK2, mV2, p);
+            mQ, mdO, mK1, mV1, mK2, mV2, mAK1, mAV1, mAK2, mAV2, p);
     }
     PF_CUDA(ctx, cudaGetLastError());
     ctx->n_launches += 1;
-    {
-        const int64_t threads = Lq * Hq * (D / 8);
-        pf::acc_to_bf16_kernel<D><<<unsigned((threads + 255) / 256), 256, 0, s>>>(
-            dqacc, static_cast<__nv_bfloat16*>(dQ.ptr), dQ.stride_tok, dQ.stride_head, Lq, Hq,
-            g->sigma);
+    if (nQS > 0) {
+        pf::dq_finish_kernel<D><<<dim3(nQS, Hq), 256, 0, s>>>(
+            dqacc, static_cast<__nv_bfloat16*>(dQ.ptr), dQ.stride_tok, dQ.stride_head, g->sigma, seq);
         PF_CUDA(ctx, cudaGetLastError());
         ctx->n_launches += 1;
     }
@@ -401,9 +466,9 @@ const char* pf_last_error(const pf_ctx* ctx) { return ctx ? ctx->err : "pf_ctx i
 
 pf_status pf_set_option(pf_ctx* ctx, const char* name, int64_t value) {
     if (!ctx || !name) return PF_INVALID_ARG;
-    if (strcmp(name, "bwd_head_parts") == 0) {
-        if (value < 0) return fail(ctx, PF_INVALID_ARG, "bwd_head_parts must be >= 0");
-        ctx->bwd_head_parts = int(value);
+    if (strcmp(name, "bwd_pairs_per_item") == 0 || strcmp(name, "bwd_heads_per_item") == 0) {
+        if (value < 0 || value > (1 << 20)) return fail(ctx, PF_INVALID_ARG, "%s must be >= 0", name);
+        (name[4] == 'p' ? ctx->bwd_pairs_per_item : ctx->bwd_heads_per_item) = int(value);
         return PF_OK;
     }
     if (strcmp(name, "profile") == 0) {
@@ -448,8 +513,10 @@ size_t pf_workspace_bytes(const pf_desc* desc, int64_t Lp, int64_t max_Ls) {
     if (!desc || Lp < 0 || max_Ls < 0 || desc->n_q_heads <= 0 || desc->n_kv_heads <= 0 ||
         desc->head_dim <= 0)
         return 0;
+    // every sequence of a packed wave is padded to a multiple of 64 rows: room for 16 ragged tails
     const int64_t Lmax = Lp > max_Ls ? Lp : max_Ls;
-    return size_t(ws_layout(*desc, Lmax).total) + size_t(kAlign);
+    const int64_t cap = align_up(Lmax, 64) + 64 * 16;
+    return size_t(cap * ws_bytes_per_pos(*desc)) + size_t(8 * kAlign);
 }
 
 pf_status pf_group_begin(pf_ctx* ctx, const pf_desc* desc, int64_t Lp, pf_tensor K1, pf_tensor V1,
@@ -492,6 +559,7 @@ pf_status pf_group_begin(pf_ctx* ctx, const pf_desc* desc, int64_t Lp, pf_tensor
     g->gV1 = static_cast<float*>(gV1.ptr);
     g->ws = static_cast<uint8_t*>(workspace);
     g->ws_bytes = workspace_bytes;
+    g->ws_cap = ws_capacity(*desc, workspace_bytes);
     g->state = 0;
     if (g->gK1 && Lp > 0) {
         cudaStream_t s = static_cast<cudaStream_t>(stream);
@@ -587,29 +655,43 @@ pf_status pf_phaseB_bwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens
     if ((st = check_tensor(ctx, "dV2", dV2, total, Hkv, d))) return st;
     if (total > 0 && !LSE2) return fail(ctx, PF_INVALID_ARG, "LSE2 is NULL");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
-    for (int i = 0; i < n_seqs; ++i) {
-        const int64_t t0 = cu_seqlens_host[i], Ls = cu_seqlens_host[i + 1] - t0;
-        if (Ls == 0) continue;
-        const WsLayout w = ws_layout(grp->desc, Ls);
-        if (size_t(w.total) > grp->ws_bytes)
-            return fail(ctx, PF_WORKSPACE, "workspace too small for a suffix of %lld tokens", (long long)Ls);
-        float* ak = reinterpret_cast<float*>(grp->ws + w.off_ak);
-        float* av = reinterpret_cast<float*>(grp->ws + w.off_av);
-        const size_t kvb = size_t(Ls) * Hkv * d * 4;
+    const WsLayout w = ws_layout(grp->desc, grp->ws_cap);
+    float* ak = reinterpret_cast<float*>(grp->ws + w.off_ak);
+    float* av = reinterpret_cast<float*>(grp->ws + w.off_av);
+    // the wave is cut into launches of <= kMaxSeqs non-empty sequences that fit the workspace
+    int i = 0;
+    while (i < n_seqs) {
+        int64_t cu[pf::kMaxSeqs + 1];
+        int n = 0;
+        int64_t t0 = 0, npad = 0;
+        for (; i < n_seqs && n < pf::kMaxSeqs; ++i) {
+            const int64_t b = cu_seqlens_host[i], Ls = cu_seqlens_host[i + 1] - b;
+            if (Ls == 0) continue;
+            const int64_t pad = align_up(Ls, 64);
+            if (n > 0 && npad + pad > grp->ws_cap) break;
+            if (n == 0) { t0 = b; cu[0] = 0; }
+            npad += pad;
+            cu[++n] = b + Ls - t0;
+        }
+        if (n == 0) break;
+        if (npad > grp->ws_cap)
+            return fail(ctx, PF_WORKSPACE, "workspace too small for a suffix of %lld tokens", (long long)cu[1]);
+        const int64_t tot = cu[n];
+        const size_t kvb = size_t(tot) * Hkv * d * 4;
         PF_CUDA(ctx, cudaMemsetAsync(ak, 0, kvb, s));
         PF_CUDA(ctx, cudaMemsetAsync(av, 0, kvb, s));
         const pf_tensor q = tok_offset(Q2, t0), k = tok_offset(K2, t0), v = tok_offset(V2, t0),
                         o = tok_offset(O2, t0), dout = tok_offset(dO2, t0), dq = tok_offset(dQ2, t0);
         if (d == 64) {
             st = launch_bwd<64>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, dout,
-                                grp->gK1, grp->gV1, ak, av, dq, Ls, 2, s);
-            if (!st) st = launch_convert_kv<64>(grp, ak, tok_offset(dK2, t0), Ls, s);
-            if (!st) st = launch_convert_kv<64>(grp, av, tok_offset(dV2, t0), Ls, s);
+                                grp->gK1, grp->gV1, ak, av, dq, n, cu, 2, s);
+            if (!st) st = launch_convert_kv<64>(grp, ak, tok_offset(dK2, t0), tot, s);
+            if (!st) st = launch_convert_kv<64>(grp, av, tok_offset(dV2, t0), tot, s);
         } else {
             st = launch_bwd<128>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, dout,
-                                 grp->gK1, grp->gV1, ak, av, dq, Ls, 2, s);
-            if (!st) st = launch_convert_kv<128>(grp, ak, tok_offset(dK2, t0), Ls, s);
-            if (!st) st = launch_convert_kv<128>(grp, av, tok_offset(dV2, t0), Ls, s);
+                                 grp->gK1, grp->gV1, ak, av, dq, n, cu, 2, s);
+            if (!st) st = launch_convert_kv<128>(grp, ak, tok_offset(dK2, t0), tot, s);
+            if (!st) st = launch_convert_kv<128>(grp, av, tok_offset(dV2, t0), tot, s);
         }
         if (st) return st;
     }
@@ -636,8 +718,8 @@ pf_status pf_phaseC_bwd(pf_group* grp, pf_tensor Q1, pf_tensor O1, const float* 
         float* ak = grp->gK1;
         float* av = grp->gV1;
         if (!ak) {  // replay baseline: no injection, accumulate in the workspace
-            const WsLayout w = ws_layout(grp->desc, Lp);
-            if (size_t(w.total) > grp->ws_bytes) return fail(ctx, PF_WORKSPACE, "workspace too small");
+            const WsLayout w = ws_layout(grp->desc, grp->ws_cap);
+            if (align_up(Lp, 64) > grp->ws_cap) return fail(ctx, PF_WORKSPACE, "workspace too small");
             ak = reinterpret_cast<float*>(grp->ws + w.off_ak);
             av = reinterpret_cast<float*>(grp->ws + w.off_av);
             const size_t kvb = size_t(Lp) * Hkv * d * 4;
@@ -645,14 +727,15 @@ pf_status pf_phaseC_bwd(pf_group* grp, pf_tensor Q1, pf_tensor O1, const float* 
             PF_CUDA(ctx, cudaMemsetAsync(av, 0, kvb, s));
         }
         pf_tensor none = {nullptr, 0, 0};
+        const int64_t cu[2] = {0, Lp};
         if (d == 64) {
             st = launch_bwd<64>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, dO1, nullptr,
-                                nullptr, ak, av, dQ1, Lp, 3, s);
+                                nullptr, ak, av, dQ1, 1, cu, 3, s);
             if (!st) st = launch_convert_kv<64>(grp, ak, dK1, Lp, s);
             if (!st) st = launch_convert_kv<64>(grp, av, dV1, Lp, s);
         } else {
             st = launch_bwd<128>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, dO1, nullptr,
-                                 nullptr, ak, av, dQ1, Lp, 3, s);
+                                 nullptr, ak, av, dQ1, 1, cu, 3, s);
             if (!st) st = launch_convert_kv<128>(grp, ak, dK1, Lp, s);
             if (!st) st = launch_convert_kv<128>(grp, av, dV1, Lp, s);
         }

@@ -34,19 +34,39 @@ class DeviceGroup:
     dQ1: torch.Tensor = None; dK1: torch.Tensor = None; dV1: torch.Tensor = None
     workspace: torch.Tensor = None
     desc: pf.pf_desc = None
+    wave: int = 1
+    packed: list = None   # per wave: cu offsets, suffix indices and the packed tensors
 
 
-def to_device(inp, device="cuda", suffixes: Optional[Sequence[int]] = None) -> DeviceGroup:
-    """Copy a `inputs.GroupInputs` to the device and allocate every output buffer."""
+def _waves(n: int, wave: int) -> List[List[int]]:
+    b = max(1, int(wave))
+    return [list(range(i, min(n, i + b))) for i in range(0, n, b)]
+
+
+def to_device(inp, device="cuda", suffixes: Optional[Sequence[int]] = None, wave: int = 1) -> DeviceGroup:
+    """Copy a `inputs.GroupInputs` to the device and allocate every output buffer.
+
+    `wave` = b packs b consecutive suffixes back to back along the token axis (the suffix
+    microbatch of PAPER.md:158, 242); Phase B then issues one call per wave.  The per-suffix
+    entries of Q2, O2, ... are views of the packed wave tensors."""
     s = inp.shape
     idx = list(range(s.N)) if suffixes is None else list(suffixes)
     dev = torch.device(device)
     mv = lambda t: t.to(dev)
     g = DeviceGroup(
         s.n_q_heads, s.n_kv_heads, s.head_dim, s.Lp, [s.Ls[i] for i in idx],
-        mv(inp.Q1), mv(inp.K1), mv(inp.V1), mv(inp.dO1),
-        [mv(inp.Q2[i]) for i in idx], [mv(inp.K2[i]) for i in idx],
-        [mv(inp.V2[i]) for i in idx], [mv(inp.dO2[i]) for i in idx])
+        mv(inp.Q1), mv(inp.K1), mv(inp.V1), mv(inp.dO1), [], [], [], [])
+    g.wave = max(1, int(wave))
+    g.packed = []
+    for w in _waves(len(idx), g.wave):
+        cu = [0]
+        for k in w:
+            cu.append(cu[-1] + g.Ls[k])
+        pk = {"cu": cu, "idx": w}
+        for name, src in (("Q2", inp.Q2), ("K2", inp.K2), ("V2", inp.V2), ("dO2", inp.dO2)):
+            pk[name] = torch.cat([src[idx[k]] for k in w], 0).contiguous().to(dev)
+            getattr(g, name).extend(pk[name][cu[j]:cu[j + 1]] for j in range(len(w)))
+        g.packed.append(pk)
     alloc_outputs(g)
     return g
 
@@ -56,30 +76,42 @@ def alloc_outputs(g: DeviceGroup) -> None:
     bf, f32 = torch.bfloat16, torch.float32
     e = lambda L, H, dt=bf: torch.empty((L, H, g.d), dtype=dt, device=dev)
     g.O1 = e(g.Lp, g.Hq); g.LSE1 = torch.empty((g.Hq, g.Lp), dtype=f32, device=dev)
-    g.O2 = [e(L, g.Hq) for L in g.Ls]
-    g.LSE2 = [torch.empty((g.Hq, L), dtype=f32, device=dev) for L in g.Ls]
-    g.dQ2 = [e(L, g.Hq) for L in g.Ls]
-    g.dK2 = [e(L, g.Hkv) for L in g.Ls]; g.dV2 = [e(L, g.Hkv) for L in g.Ls]
+    g.O2, g.LSE2, g.dQ2, g.dK2, g.dV2 = [], [], [], [], []
+    max_tok = 0
+    for pk in g.packed:
+        cu = pk["cu"]
+        tot = cu[-1]
+        max_tok = max(max_tok, tot)
+        pk["O2"] = e(tot, g.Hq); pk["dQ2"] = e(tot, g.Hq)
+        pk["dK2"] = e(tot, g.Hkv); pk["dV2"] = e(tot, g.Hkv)
+        pk["LSE2"] = torch.empty((g.Hq, tot), dtype=f32, device=dev)
+        for j in range(len(pk["idx"])):
+            sl = slice(cu[j], cu[j + 1])
+            g.O2.append(pk["O2"][sl]); g.dQ2.append(pk["dQ2"][sl])
+            g.dK2.append(pk["dK2"][sl]); g.dV2.append(pk["dV2"][sl])
+            g.LSE2.append(pk["LSE2"][:, sl])
     g.gK1 = e(g.Lp, g.Hkv, f32); g.gV1 = e(g.Lp, g.Hkv, f32)
     g.dQ1 = e(g.Lp, g.Hq); g.dK1 = e(g.Lp, g.Hkv); g.dV1 = e(g.Lp, g.Hkv)
     g.desc = pf.make_desc(g.Hq, g.Hkv, g.d)
-    nbytes = pf.pf_workspace_bytes(g.desc, g.Lp, max(g.Ls, default=0))
+    nbytes = pf.pf_workspace_bytes(g.desc, g.Lp, max_tok)
     g.workspace = torch.empty(nbytes, dtype=torch.uint8, device=dev)
 
 
 def run_prefixflow_step(ctx, g: DeviceGroup, stream=None, after_each_suffix=None,
                         order: Optional[Sequence[int]] = None) -> None:
-    """Phase A -> Phase B (fwd, bwd) per suffix -> Phase C."""
+    """Phase A -> Phase B (fwd, bwd) per suffix wave -> Phase C.
+    `order` permutes the waves (= the suffixes when wave == 1)."""
     grp = pf.pf_group_begin(ctx, g.desc, g.Lp, g.K1, g.V1, g.gK1, g.gV1, g.workspace, stream)
     try:
         pf.pf_phaseA_fwd(grp, g.Q1, g.O1, g.LSE1, stream)
-        for i in (range(len(g.Ls)) if order is None else order):
-            cu = [0, g.Ls[i]]
-            pf.pf_phaseB_fwd(grp, cu, g.Q2[i], g.K2[i], g.V2[i], g.O2[i], g.LSE2[i], stream)
-            pf.pf_phaseB_bwd(grp, cu, g.Q2[i], g.K2[i], g.V2[i], g.O2[i], g.LSE2[i], g.dO2[i],
-                             g.dQ2[i], g.dK2[i], g.dV2[i], stream)
+        for i in (range(len(g.packed)) if order is None else order):
+            pk = g.packed[i]
+            cu = pk["cu"]
+            pf.pf_phaseB_fwd(grp, cu, pk["Q2"], pk["K2"], pk["V2"], pk["O2"], pk["LSE2"], stream)
+            pf.pf_phaseB_bwd(grp, cu, pk["Q2"], pk["K2"], pk["V2"], pk["O2"], pk["LSE2"], pk["dO2"],
+                             pk["dQ2"], pk["dK2"], pk["dV2"], stream)
             if after_each_suffix is not None:
-                after_each_suffix(i)
+                after_each_suffix(pk["idx"][-1])
         pf.pf_phaseC_bwd(grp, g.Q1, g.O1, g.LSE1, g.dO1, g.dQ1, g.dK1, g.dV1, stream)
     finally:
         pf.pf_group_end(grp)

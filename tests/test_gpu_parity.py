@@ -21,25 +21,27 @@ def ctx():
     pf.pf_destroy(c)
 
 
-def run_and_compare(ctx, shape, weights=None, order=None, zero_dO1=False, parts=None):
+def run_and_compare(ctx, shape, weights=None, order=None, zero_dO1=False, items=None, wave=1):
     inp = inputs.make_group(shape)
     if zero_dO1:
         inp.dO1.zero_()
     ref = oracle.group_reference(inp, weights=weights, order=order)
-    g = schedule.to_device(inp)
+    g = schedule.to_device(inp, wave=wave)
     snaps = {}
 
     def snap(i):
         snaps[i] = (g.gK1.clone(), g.gV1.clone())
 
-    if parts is not None:
-        pf.pf_set_option(ctx, "bwd_head_parts", parts)
+    if items is not None:
+        pf.pf_set_option(ctx, "bwd_pairs_per_item", items[0])
+        pf.pf_set_option(ctx, "bwd_heads_per_item", items[1])
     try:
         schedule.run_prefixflow_step(ctx, g, after_each_suffix=snap, order=order)
         torch.cuda.synchronize()
     finally:
-        if parts is not None:
-            pf.pf_set_option(ctx, "bwd_head_parts", 0)
+        if items is not None:
+            pf.pf_set_option(ctx, "bwd_pairs_per_item", 0)
+            pf.pf_set_option(ctx, "bwd_heads_per_item", 0)
     return g, ref, compare_group(g, ref, snaps)
 
 
@@ -75,10 +77,37 @@ def test_smallest_nonempty(ctx):
     run_and_compare(ctx, inputs.small_case(1, 1, 128, 1, [1], seed=11, dist="std"))
 
 
-@pytest.mark.parametrize("parts", [1, 2, 7])
-def test_bwd_head_parts(ctx, parts):
-    """gK1/gV1 accumulation with the KV tile owned by one CTA (no contention) or split over heads."""
-    run_and_compare(ctx, inputs.small_case(7, 1, 128, 260, [140, 70], seed=5, dist="unit"), parts=parts)
+@pytest.mark.parametrize("items", [(1, 1), (2, 3), (7, 7), (1000, 1000)])
+@pytest.mark.parametrize("wave", [1, 2])
+def test_bwd_item_sizes(ctx, items, wave):
+    """gK1/gV1 accumulation with a key tile owned by one CTA (no contention) or split over
+    (sequence, head) pairs: `items` = (pairs per prefix-tile CTA, heads per causal-tile CTA)."""
+    run_and_compare(ctx, inputs.small_case(7, 1, 128, 260, [140, 70], seed=5, dist="unit"),
+                    items=items, wave=wave)
+
+
+@pytest.mark.parametrize("Hq,Hkv,d,Lp,Ls,wave", [
+    (4, 2, 128, 300, [129, 64, 1, 200], 4),     # one packed wave, ragged tails, Ls = 1 inside
+    (7, 1, 64, 130, [65, 0, 127, 64, 3], 3),    # d = 64, an empty suffix inside a wave, 2 waves
+    (2, 2, 128, 0, [70, 130, 64], 3),           # Lp = 0: packed plain causal attention
+    (4, 1, 128, 129, [63] * 5, 5),              # equal short suffixes
+])
+@pytest.mark.parametrize("dist", ["std", "unit"])
+def test_packed_waves(ctx, Hq, Hkv, d, Lp, Ls, wave, dist):
+    """Packed suffix microbatches: n_seqs > 1 per Phase-B call; gK1/gV1 are
+    compared after every wave, everything else per suffix."""
+    run_and_compare(ctx, inputs.small_case(Hq, Hkv, d, Lp, Ls, seed=23, dist=dist), wave=wave)
+
+
+def test_wave_split_by_workspace(ctx):
+    """A wave whose padded length exceeds the workspace is cut into several launches."""
+    shape = inputs.small_case(2, 1, 64, 64, [100] * 40, seed=29, dist="unit")   # 40 > kMaxSeqs = 32
+    inp = inputs.make_group(shape)
+    ref = oracle.group_reference(inp)
+    g = schedule.to_device(inp, wave=40)
+    schedule.run_prefixflow_step(ctx, g)
+    torch.cuda.synchronize()
+    compare_group(g, ref)
 
 
 def test_degenerate_lengths(ctx):
@@ -134,7 +163,8 @@ def test_strided_inputs(ctx):
         buf[:, :Hq] = q; buf[:, Hq:Hq + Hkv] = k; buf[:, Hq + Hkv:] = v
         return buf[:, :Hq], buf[:, Hq:Hq + Hkv], buf[:, Hq + Hkv:]
     g.Q1, g.K1, g.V1 = fuse(g.Q1, g.K1, g.V1)
-    g.Q2[0], g.K2[0], g.V2[0] = fuse(g.Q2[0], g.K2[0], g.V2[0])
+    pk = g.packed[0]
+    pk["Q2"], pk["K2"], pk["V2"] = fuse(pk["Q2"], pk["K2"], pk["V2"])
     assert not g.Q1.is_contiguous()
     schedule.run_prefixflow_step(ctx, g)
     torch.cuda.synchronize()
