@@ -251,12 +251,15 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 const uint64_t dQ_k = make_smem_desc_sw128(smem_u32(smem + C::OFF_Q + st * C::QTILE), 16, 1024);
                 const uint64_t ddO_k = make_smem_desc_sw128(smem_u32(smem + C::OFF_DO + st * C::QTILE), 16, 1024);
                 mbar_wait(&bar_Qf[st], (it / C::QS) & 1);
-                if (it >= 2) mbar_wait(&bar_dQfree[b], ((it >> 1) - 1) & 1);  // dP^T region held dQ^T
                 tc_fence_after();
 #pragma unroll
                 for (int kk = 0; kk < D / 16; ++kk)   // S^T = K Q^T
                     mma_ss(tmem + T_S + b * 64, dK_k + (((kk >> 2) * C::KSUB + (kk & 3) * 32) >> 4),
                            dQ_k + (((kk >> 2) * C::QSUB + (kk & 3) * 32) >> 4), id_s, kk > 0);
+                if (it >= 2) {                        // the dP^T region still holds dQ^T(it - 2)
+                    mbar_wait(&bar_dQfree[b], ((it >> 1) - 1) & 1);
+                    tc_fence_after();
+                }
 #pragma unroll
                 for (int kk = 0; kk < D / 16; ++kk)   // dP^T = V dO^T
                     mma_ss(tmem + T_DP + b * 64, dV_k + (((kk >> 2) * C::KSUB + (kk & 3) * 32) >> 4),
@@ -273,7 +276,6 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 const uint32_t sdS = smem_u32(smem + C::OFF_DS + b * C::DSB);
                 const uint64_t dQ_mn = make_smem_desc_sw128(sQ, C::QSUB, 1024);
                 const uint64_t ddO_mn = make_smem_desc_sw128(sdO, C::QSUB, 1024);
-                const uint64_t ddS_k = make_smem_desc_sw128(sdS, 16, 1024);
                 const uint64_t ddS_mn = make_smem_desc_sw128(sdS, C::DSB, 1024);
                 mbar_wait(&bar_P[b], (it >> 1) & 1);
                 tc_fence_after();
@@ -287,9 +289,9 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     mma_ts(tmem + T_DV, tmem + T_S + b * 64 + (kk >> 1) * 32 + (kk & 1) * 8,
                            ddO_mn + ((kk * 2048) >> 4), id_kv, (it > 0 || kk > 0) ? 1u : 0u);
 #pragma unroll
-                for (int kk = 0; kk < 4; ++kk)  // dK += dS^T Q  (A = dS^T K-major, B = Q MN-major)
-                    mma_ss(tmem + T_DK, ddS_k + ((kk * 32) >> 4), dQ_mn + ((kk * 2048) >> 4), id_kv,
-                           (it > 0 || kk > 0) ? 1u : 0u);
+                for (int kk = 0; kk < 4; ++kk)  // dK += dS^T Q  (A from TMEM, B = Q MN-major)
+                    mma_ts(tmem + T_DK, tmem + T_S + b * 64 + (kk >> 1) * 32 + 16 + (kk & 1) * 8,
+                           dQ_mn + ((kk * 2048) >> 4), id_kv, (it > 0 || kk > 0) ? 1u : 0u);
                 mma_commit(&bar_Qe[st]);
             }
             mma_commit(bar_done);
@@ -298,51 +300,65 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         // =============================== compute warpgroups ===============================
         if (n_iter > 0) {
             const int w = warp >> 2;                             // query-column half
-            const int j = tid & 127;                             // key row in tile == TMEM lane
+            const int j = tid & 127;                             // key row in tile == TMEM lane (epilogue)
             const uint32_t lane_off = uint32_t((warp & 3) * 32) << 16;
-            const int kj = kt * 128 + j;                         // key index within its sequence
+            // Fragment layout of tcgen05.ld/st .16x256b / .16x128b (one instruction = 16 TMEM lanes):
+            // thread l holds, for half hf in {0,1} and column group r in 0..3, key row
+            // 16 blk + 8 hf + l/4 and the query-column pair 8 r + 2 (l%4) + {0,1} of its 32 columns,
+            // so it needs only 8 of the 64 per-column statistics (2 x 4 LDS.64 per iteration).
+            const int lane = tid & 31, lq = lane & 3, lr = lane >> 2;
+            const uint32_t tS_w = tmem + T_S + w * 32 + lane_off, tDP_w = tmem + T_DP + w * 32 + lane_off;
             BwdIter iter(p, pair_lo, pair_hi, g, qs_lo);
             for (int it = 0; iter.valid(); ++it, iter.next()) {
                 const int st = it % C::QS, b = it & 1;
-                const float4* s_lse = reinterpret_cast<const float4*>(smem + C::OFF_STAT + st * 512) + w * 8;
-                const float4* s_dl = s_lse + 16;
-                uint8_t* dsrow = smem + C::OFF_DS + b * C::DSB + j * 128;
+                const float2* s_lse = reinterpret_cast<const float2*>(smem + C::OFF_STAT + st * 512) + w * 16 + lq;
+                const float2* s_dl = s_lse + 32;
+                uint8_t* ds_tile = smem + C::OFF_DS + b * C::DSB;
                 mbar_wait(&bar_Qf[st], (it / C::QS) & 1);        // lse2 / delta visible
+                float2 lv[4], dv[4];
+#pragma unroll
+                for (int r = 0; r < 4; ++r) { lv[r] = s_lse[r * 4]; dv[r] = s_dl[r * 4]; }
                 mbar_wait(&bar_S[b], (it >> 1) & 1);
                 tc_fence_after();
-                uint32_t s[32], dp[32];
-                tmem_ld32(tmem + T_S + b * 64 + w * 32 + lane_off, s);
-                tmem_ld32(tmem + T_DP + b * 64 + w * 32 + lane_off, dp);
+                uint32_t s[2][16], dp[2][16];
+#pragma unroll
+                for (int blk = 0; blk < 2; ++blk) {
+                    tmem_ld_16x256b_x4(tS_w + b * 64 + (uint32_t(blk * 16) << 16), s[blk]);
+                    tmem_ld_16x256b_x4(tDP_w + b * 64 + (uint32_t(blk * 16) << 16), dp[blk]);
+                }
                 tmem_wait_ld();
                 // causal source: query t sees key kj iff t >= kj; only diagonal sub-tiles need it
                 const bool diag = !pre && iter.qs * 64 < kt * 128 + 128;
-                const int first = kj - (iter.qs * 64 + w * 32);  // local columns < first are masked
-                uint32_t pk[16], dsk[16];
+                const int col0 = iter.qs * 64 + w * 32 + 2 * lq;  // query (within its sequence) of r = 0, e = 0
 #pragma unroll
-                for (int q4 = 0; q4 < 8; ++q4) {
-                    const float4 l = s_lse[q4], dl = s_dl[q4];
-                    const float lv[4] = {l.x, l.y, l.z, l.w}, dv[4] = {dl.x, dl.y, dl.z, dl.w};
-                    float pv[4], dsv[4];
+                for (int blk = 0; blk < 2; ++blk) {
+                    uint32_t pk[8], dsk[8];
 #pragma unroll
-                    for (int e = 0; e < 4; ++e) {
-                        const int q = q4 * 4 + e;
-                        float pe = fast_exp2(fmaf(__uint_as_float(s[q]), p.scale_log2, -lv[e]));
-                        if (diag && q < first) pe = 0.f;
-                        pv[e] = pe;
-                        dsv[e] = pe * (__uint_as_float(dp[q]) - dv[e]);
+                    for (int hf = 0; hf < 2; ++hf) {
+                        const int row = (warp & 3) * 32 + blk * 16 + hf * 8 + lr;   // key row in tile
+                        const int kj = kt * 128 + row;
+#pragma unroll
+                        for (int r = 0; r < 4; ++r) {
+                            const int i = r * 4 + hf * 2;
+                            float p0 = fast_exp2(fmaf(__uint_as_float(s[blk][i]), p.scale_log2, -lv[r].x));
+                            float p1 = fast_exp2(fmaf(__uint_as_float(s[blk][i + 1]), p.scale_log2, -lv[r].y));
+                            if (diag) {
+                                if (col0 + 8 * r < kj) p0 = 0.f;
+                                if (col0 + 8 * r + 1 < kj) p1 = 0.f;
+                            }
+                            const float d0 = p0 * (__uint_as_float(dp[blk][i]) - dv[r].x);
+                            const float d1 = p1 * (__uint_as_float(dp[blk][i + 1]) - dv[r].y);
+                            pk[r * 2 + hf] = pack_bf16(p0, p1);
+                            const uint32_t dsv = pack_bf16(d0, d1);
+                            dsk[r * 2 + hf] = dsv;
+                            // dS^T -> smem, K-major swizzle-128B tile [128 keys][64 queries]
+                            *reinterpret_cast<uint32_t*>(ds_tile + row * 128 + (((w * 4 + r) ^ (row & 7)) << 4) + lq * 4) = dsv;
+                        }
                     }
-                    pk[q4 * 2] = pack_bf16(pv[0], pv[1]);
-                    pk[q4 * 2 + 1] = pack_bf16(pv[2], pv[3]);
-                    dsk[q4 * 2] = pack_bf16(dsv[0], dsv[1]);
-                    dsk[q4 * 2 + 1] = pack_bf16(dsv[2], dsv[3]);
+                    // P^T and dS^T -> TMEM (bf16 pairs): columns [0,16) and [16,32) of this half's S^T
+                    tmem_st_16x128b_x4(tS_w + b * 64 + (uint32_t(blk * 16) << 16), pk);
+                    tmem_st_16x128b_x4(tS_w + b * 64 + 16 + (uint32_t(blk * 16) << 16), dsk);
                 }
-                // P^T -> TMEM (bf16 pairs) over the first 16 columns of this half's S^T region
-                tmem_st16(tmem + T_S + b * 64 + w * 32 + lane_off, pk);
-                // dS^T -> smem, K-major swizzle-128B tile [128 keys][64 queries]
-#pragma unroll
-                for (int ch = 0; ch < 4; ++ch)
-                    *reinterpret_cast<uint4*>(dsrow + (((w * 4 + ch) ^ (j & 7)) << 4)) =
-                        make_uint4(dsk[ch * 4], dsk[ch * 4 + 1], dsk[ch * 4 + 2], dsk[ch * 4 + 3]);
                 tmem_wait_st();
                 fence_proxy_async_smem();
                 tc_fence_before();
@@ -385,15 +401,14 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 float* dst = p.dQacc + (int64_t(iter.h) * p.nQS + iter.qsg0 + iter.qs) * (2 * D * 32);
                 mbar_wait(&bar_dQ[b], (it >> 1) & 1);
                 tc_fence_after();
+                uint32_t v[2][32];
+                tmem_ld32(tmem + T_DP + b * 64 + lane_off, v[0]);
+                tmem_ld32(tmem + T_DP + b * 64 + 32 + lane_off, v[1]);
+                tmem_wait_ld();
+                tc_fence_before();
+                mbar_arrive(&bar_dQfree[b]);                     // TMEM buffer free for dP^T(it + 2)
 #pragma unroll
                 for (int half = 0; half < 2; ++half) {
-                    uint32_t v[32];
-                    tmem_ld32(tmem + T_DP + b * 64 + half * 32 + lane_off, v);
-                    tmem_wait_ld();
-                    if (half == 1) {
-                        tc_fence_before();
-                        mbar_arrive(&bar_dQfree[b]);
-                    }
                     uint8_t* stage = smem + C::OFF_DQ + half * C::DQB;
                     if (dl == 0) bulk_wait_read<1>();            // this buffer's previous reduce has read it
                     named_bar_sync(3, 128);
@@ -401,7 +416,8 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 #pragma unroll
                         for (int ch = 0; ch < 8; ++ch)
                             *reinterpret_cast<uint4*>(stage + dl * 128 + ((ch ^ (dl & 7)) << 4)) =
-                                make_uint4(v[ch * 4], v[ch * 4 + 1], v[ch * 4 + 2], v[ch * 4 + 3]);
+                                make_uint4(v[half][ch * 4], v[half][ch * 4 + 1], v[half][ch * 4 + 2],
+                                           v[half][ch * 4 + 3]);
                     }
                     fence_proxy_async_smem();
                     named_bar_sync(4, 128);
