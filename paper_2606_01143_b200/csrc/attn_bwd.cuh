@@ -29,18 +29,9 @@
 #pragma once
 #include <cuda.h>
 #include "sm100_ptx.cuh"
+#include "seq_table.cuh"
 
 namespace pf {
-
-constexpr int kMaxSeqs = 32;  // sequences per launch (the host splits longer waves)
-
-// Sequences of one launch: packed back to back along the token axis.
-struct SeqTable {
-    int n;
-    int cu[kMaxSeqs + 1];   // token offset of sequence s in the packed tensors
-    int pqs[kMaxSeqs + 1];  // prefix sums of ceil(Ls / 64): first global query sub-tile of s
-    int ckt[kMaxSeqs + 1];  // prefix sums of ceil(Ls / 128): first global causal key tile of s
-};
 
 struct BwdParams {
     float* dQacc;                  // [Hq][nQS][2][D][32] fp32 tiles (16-B chunks xor-swizzled by d&7)

@@ -8,7 +8,7 @@
 #include <cuda_runtime.h>
 #include <cuda_bf16.h>
 #include <stdint.h>
-#include "attn_bwd.cuh"  // SeqTable
+#include "seq_table.cuh"
 
 namespace pf {
 
