@@ -1,35 +1,39 @@
-// attn_fwd.cuh -- sm_100a attention forward with two KV sources.
+// attn_fwd.cuh -- sm_100a attention forward with two KV sources, packed sequences.
 //
 //   O[t,h] = softmax_j( sigma <q[h,t], k[g,j]> ) v[g,j],   LSE[h,t] = log sum_j exp(sigma <q,k>)
 //
 // KV source 1 ("prefix", length Lp): every key is visible to every query (cached K1/V1, read in
-// place -- no concat copy).  KV source 2 ("causal", same length as the queries): key j visible to
-// query t iff j <= t.  Phase A / replay: Lp = 0.  Phase B: source 1 = cached prefix.
+// place -- no concat copy).  KV source 2 ("causal"): the keys of the query's own sequence, key j
+// visible to query t iff j <= t.  Phase A / replay: Lp = 0, one sequence.  Phase B: source 1 = the
+// cached prefix, the sequences are the suffixes of the wave packed along the token axis.
 //
 // One CTA = two query tiles of 128 rows ("slots": consecutive (row block, q head) items of one KV
-// head, so both read the same K/V stream) ping-ponged on the tensor core:
+// head and one sequence, so both read the same K/V stream) ping-ponged on the tensor core:
 //   warps 0-3  softmax of slot 0   (thread r <-> query row r <-> TMEM lane r)
 //   warps 4-7  softmax of slot 1
 //   warp  8    TMA producer (Q once, K/V tiles through a 2-stage ring)
 //   warp  9    tcgen05.mma issuer (one thread)
 // TMEM (512 columns): S0 | S1 | O0 | O1, 128 fp32 columns each; P (bf16) overwrites the first 64
-// columns of its S and is consumed from TMEM as the A operand of P.V.
+// columns of its S and is consumed from TMEM as the A operand of P.V, handed over in two halves
+// (keys 0-63, 64-127) so that P.V starts while the second half is still being exponentiated.
+// A quarter of the exponentials is evaluated by a degree-3 polynomial on the FMA pipe, the rest by
+// MUFU.EX2 (16 / clk / SM, which alone would tie with the tensor pipe).
 #pragma once
 #include <cuda.h>
 #include "sm100_ptx.cuh"
+#include "seq_table.cuh"
 
 namespace pf {
 
 struct FwdParams {
     __nv_bfloat16* O;
     int64_t o_stride_tok, o_stride_head;  // elements
-    float* LSE;                           // [Hq, lse_stride]
+    float* LSE;                           // [Hq, lse_stride], column = packed token row
     int64_t lse_stride;
-    int Lq;        // queries (= causal-source keys)
     int Lp;        // prefix-source keys (0: none)
     int Hq, Hkv, G;
-    int nRB;       // ceil(Lq / 128)
     float scale_log2;  // sigma * log2(e)
+    SeqTable seq;
 };
 
 template <int D>
@@ -46,11 +50,29 @@ struct FwdCfg {
     static constexpr int THREADS = 320;
 };
 
+// 2^x for a pair of x <= ~8 on the FMA / ALU pipes (packed f32x2 math): round-to-nearest split
+// x = j + f, |f| <= 1/2, degree-3 minimax polynomial for 2^f (max relative error 7.5e-5, far below
+// the bf16 rounding of P), and the exponent added with an integer shift-add.  x is clamped at -126
+// (result ~ 1e-38, i.e. 0 for P).  Finite inputs only.
+__device__ __forceinline__ float2 exp2_poly2(float2 x) {
+    x.x = fmaxf(x.x, -126.f);
+    x.y = fmaxf(x.y, -126.f);
+    const float2 magic = make_float2(12582912.f, 12582912.f);   // 1.5 * 2^23: integer in the low mantissa bits
+    const float2 t = __fadd2_rn(x, magic);
+    const float2 f = __fadd2_rn(x, __fadd2_rn(make_float2(12582912.f, 12582912.f), make_float2(-t.x, -t.y)));
+    float2 r = __ffma2_rn(f, make_float2(0.05517164617776871f, 0.05517164617776871f),
+                          make_float2(0.2426111251115799f, 0.2426111251115799f));
+    r = __ffma2_rn(r, f, make_float2(0.6932609677314758f, 0.6932609677314758f));
+    r = __ffma2_rn(r, f, make_float2(0.9999280571937561f, 0.9999280571937561f));
+    return make_float2(__int_as_float(__float_as_int(r.x) + (__float_as_int(t.x) << 23)),
+                       __int_as_float(__float_as_int(r.y) + (__float_as_int(t.y) << 23)));
+}
+
 template <int D>
 __global__ void __launch_bounds__(320, 1)
 attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK1,
                 const __grid_constant__ CUtensorMap tmV1, const __grid_constant__ CUtensorMap tmK2,
-                const __grid_constant__ CUtensorMap tmV2, const FwdParams p) {
+                const __grid_constant__ CUtensorMap tmV2, const __grid_constant__ FwdParams p) {
     using C = FwdCfg<D>;
     extern __shared__ __align__(1024) uint8_t smem[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::OFF_BAR);
@@ -60,17 +82,26 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     uint64_t* bar_Vf = bars + 6;
     uint64_t* bar_Ve = bars + 8;
     uint64_t* bar_S = bars + 10;            // [2] S_s ready (MMA -> softmax)
-    uint64_t* bar_P = bars + 12;            // [2] P_s ready (softmax -> MMA)
-    uint64_t* bar_done = bars + 14;         // all MMAs complete
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 16);
+    uint64_t* bar_P = bars + 12;            // [2 slots][2 halves] P_s half ready (softmax -> MMA)
+    uint64_t* bar_done = bars + 16;         // all MMAs complete
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 17);
 
     const int tid = threadIdx.x, warp = tid >> 5;
     if ((smem_u32(smem) & 1023u) != 0) __trap();
 
-    // ---- work decode: items of KV head g are (rb, h') with index rb*G + h'; heaviest first ----
+    // ---- work decode: sequence, then its items (rb, h') of KV head g with index rb*G + h',
+    // heaviest (largest rb) first; the two slots of a CTA are consecutive items of one sequence
     const int g = blockIdx.y;
-    const int nItems = p.nRB * p.G;
-    const int idx0 = nItems - 1 - 2 * int(blockIdx.x);
+    int sq = 0, base = 0, nRB = 0;
+    for (;; ++sq) {
+        nRB = p.seq.ckt[sq + 1] - p.seq.ckt[sq];
+        const int ncta = (nRB * p.G + 1) >> 1;
+        if (int(blockIdx.x) < base + ncta || sq + 1 >= p.seq.n) break;
+        base += ncta;
+    }
+    const int tok0 = p.seq.cu[sq], Ls = p.seq.cu[sq + 1] - tok0;
+    const int nItems = nRB * p.G;
+    const int idx0 = nItems - 1 - 2 * (int(blockIdx.x) - base);
     const int idx1 = idx0 - 1;                       // < 0: slot 1 idle
     const int rb0 = idx0 / p.G, h0 = g * p.G + idx0 % p.G;
     const int rb1 = idx1 >= 0 ? idx1 / p.G : -1, h1 = idx1 >= 0 ? g * p.G + idx1 % p.G : 0;
@@ -85,7 +116,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             mbar_init(&bar_Vf[s], 1); mbar_init(&bar_Ve[s], 1);
         }
         mbar_init(&bar_S[0], 1); mbar_init(&bar_S[1], 1);
-        mbar_init(&bar_P[0], 128); mbar_init(&bar_P[1], 128);
+        for (int i = 0; i < 4; ++i) mbar_init(&bar_P[i], 128);
         mbar_init(bar_done, 1);
         fence_mbar_init();
     }
@@ -106,18 +137,18 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         if (elect_one()) {
             mbar_arrive_expect_tx(&bar_Q[0], C::TILE);
             for (int k = 0; k < C::NSUB; ++k)
-                tma_load_3d(smem + C::OFF_Q + k * C::SUB, &tmQ, &bar_Q[0], 64 * k, h0, rb0 * 128);
+                tma_load_3d(smem + C::OFF_Q + k * C::SUB, &tmQ, &bar_Q[0], 64 * k, h0, tok0 + rb0 * 128);
             if (idx1 >= 0) {
                 mbar_arrive_expect_tx(&bar_Q[1], C::TILE);
                 for (int k = 0; k < C::NSUB; ++k)
                     tma_load_3d(smem + C::OFF_Q + C::TILE + k * C::SUB, &tmQ, &bar_Q[1], 64 * k, h1,
-                                rb1 * 128);
+                                tok0 + rb1 * 128);
             }
             for (int it = 0; it < n_iter0; ++it) {
                 const int st = it % C::KS;
                 const uint32_t ph = (it / C::KS) & 1;
                 const bool pre = it < nP;
-                const int row0 = (pre ? it : it - nP) * 128;
+                const int row0 = pre ? it * 128 : tok0 + (it - nP) * 128;
                 mbar_wait(&bar_Ke[st], ph ^ 1);
                 mbar_arrive_expect_tx(&bar_Kf[st], C::TILE);
                 for (int k = 0; k < C::NSUB; ++k)
@@ -138,20 +169,19 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             const uint32_t sQ = smem_u32(smem + C::OFF_Q), sK = smem_u32(smem + C::OFF_K),
                            sV = smem_u32(smem + C::OFF_V);
             auto issue_S = [&](int s, int st) {  // S_s = Q_s . K^T
-                const uint32_t q = sQ + s * C::TILE, k = sK + st * C::TILE;
+                const uint64_t q = make_smem_desc_sw128(sQ + s * C::TILE, 16, 1024);
+                const uint64_t k = make_smem_desc_sw128(sK + st * C::TILE, 16, 1024);
 #pragma unroll
                 for (int kk = 0; kk < D / 16; ++kk) {
-                    const uint32_t off = (kk >> 2) * C::SUB + (kk & 3) * 32;
-                    mma_ss(tmem + s * 128, make_smem_desc_sw128(q + off, 16, 1024),
-                           make_smem_desc_sw128(k + off, 16, 1024), idesc_qk, kk > 0);
+                    const uint32_t off = ((kk >> 2) * C::SUB + (kk & 3) * 32) >> 4;
+                    mma_ss(tmem + s * 128, q + off, k + off, idesc_qk, kk > 0);
                 }
             };
-            auto issue_PV = [&](int s, int st, bool acc) {  // O_s += P_s . V
-                const uint32_t v = sV + st * C::TILE;
+            auto issue_PV = [&](int s, int st, int half, bool acc) {  // O_s += P_s[:, half] . V[half]
+                const uint64_t v = make_smem_desc_sw128(sV + st * C::TILE, C::SUB, 1024);
 #pragma unroll
-                for (int kk = 0; kk < 8; ++kk)
-                    mma_ts(tmem + 256 + s * D, tmem + s * 128 + kk * 8,
-                           make_smem_desc_sw128(v + kk * 2048, C::SUB, 1024), idesc_pv,
+                for (int kk = half * 4; kk < half * 4 + 4; ++kk)
+                    mma_ts(tmem + 256 + s * D, tmem + s * 128 + kk * 8, v + ((kk * 2048) >> 4), idesc_pv,
                            (acc || kk > 0) ? 1u : 0u);
             };
             mbar_wait(&bar_Q[0], 0);
@@ -175,7 +205,10 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 mbar_wait(&bar_Vf[st], ph);
                 mbar_wait(&bar_P[0], it & 1);
                 tc_fence_after();
-                issue_PV(0, st, it > 0);
+                issue_PV(0, st, 0, it > 0);
+                mbar_wait(&bar_P[1], it & 1);
+                tc_fence_after();
+                issue_PV(0, st, 1, true);
                 if (next) {
                     mbar_wait(&bar_Kf[st1], ph1);
                     tc_fence_after();
@@ -183,9 +216,12 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     mma_commit(&bar_S[0]);
                 }
                 if (it < n_iter1) {
-                    mbar_wait(&bar_P[1], it & 1);
+                    mbar_wait(&bar_P[2], it & 1);
                     tc_fence_after();
-                    issue_PV(1, st, it > 0);
+                    issue_PV(1, st, 0, it > 0);
+                    mbar_wait(&bar_P[3], it & 1);
+                    tc_fence_after();
+                    issue_PV(1, st, 1, true);
                 }
                 mma_commit(&bar_Ve[st]);
                 if (next) {
@@ -205,83 +241,100 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         const int n_iter = s == 0 ? n_iter0 : n_iter1;
         const int rb = s == 0 ? rb0 : rb1;
         const int h = s == 0 ? h0 : h1;
-        const int t = rb * 128 + r;              // global query row
+        const int t = rb * 128 + r;              // query row within its sequence
         const uint32_t lane_off = uint32_t((warp & 3) * 32) << 16;
         const uint32_t tS = tmem + s * 128 + lane_off;
         const uint32_t tO = tmem + 256 + s * D + lane_off;
+        const float c = p.scale_log2;
         float m_used = -INFINITY, l = 0.f;
         for (int it = 0; it < n_iter; ++it) {
             mbar_wait(&bar_S[s], it & 1);
             tc_fence_after();
-            uint32_t x[4][32];
-            tmem_ld32(tS + 0, x[0]);
-            tmem_ld32(tS + 32, x[1]);
-            tmem_ld32(tS + 64, x[2]);
-            tmem_ld32(tS + 96, x[3]);
-            tmem_wait_ld();
-            int limit;
-            if (it < nP) limit = p.Lp - it * 128;
-            else limit = t - (it - nP) * 128 + 1;
-            if (limit < 128) {  // ragged prefix tail or causal diagonal
+            const int limit = it < nP ? p.Lp - it * 128 : t - (it - nP) * 128 + 1;
+            const bool masked = limit < 128;     // ragged prefix tail or causal diagonal
+            // ---- pass 1: row maximum (S is read from TMEM twice to keep the live registers low)
+            float mx0 = -INFINITY, mx1 = -INFINITY;
 #pragma unroll
-                for (int c = 0; c < 4; ++c)
+            for (int q = 0; q < 4; ++q) {
+                uint32_t x[32];
+                tmem_ld32(tS + q * 32, x);
+                tmem_wait_ld();
+                if (masked) {
 #pragma unroll
                     for (int j = 0; j < 32; ++j)
-                        if (c * 32 + j >= limit) x[c][j] = 0xff800000u;  // -inf
+                        if (q * 32 + j >= limit) x[j] = 0xf149f2cau;  // -1e30: exp2 -> 0, stays finite
+                }
+#pragma unroll
+                for (int j = 0; j < 32; j += 2) {
+                    mx0 = fmaxf(mx0, __uint_as_float(x[j]));
+                    mx1 = fmaxf(mx1, __uint_as_float(x[j + 1]));
+                }
             }
-            float mx = -INFINITY;
-#pragma unroll
-            for (int c = 0; c < 4; ++c)
-#pragma unroll
-                for (int j = 0; j < 32; ++j) mx = fmaxf(mx, __uint_as_float(x[c][j]));
-            const float m_new = mx * p.scale_log2;
+            const float m_new = fmaxf(mx0, mx1) * c;
             // lazy rescale: keep a stale max while the new one is within 2^8 of it
             const bool need = (it == 0) || (m_new > m_used + 8.f);
             if (__any_sync(0xffffffffu, need && it > 0)) {
                 const float alpha = need ? fast_exp2(m_used - m_new) : 1.f;
                 l *= alpha;
 #pragma unroll
-                for (int c = 0; c < D / 32; ++c) {
+                for (int q = 0; q < D / 32; ++q) {
                     uint32_t o[32];
-                    tmem_ld32(tO + c * 32, o);
+                    tmem_ld32(tO + q * 32, o);
                     tmem_wait_ld();
 #pragma unroll
                     for (int j = 0; j < 32; ++j) o[j] = __float_as_uint(__uint_as_float(o[j]) * alpha);
-                    tmem_st32(tO + c * 32, o);
+                    tmem_st32(tO + q * 32, o);
                 }
             }
             if (need) m_used = m_new;
-            float sum = 0.f;
+            // ---- pass 2: P = exp2(c S - m), packed to bf16 over the first 64 columns of S.  Chunk q
+            // (S columns [32q, 32q+32)) writes P columns [16q, 16q+16): always behind the reads.
+            const float2 c2 = make_float2(c, c), nm2 = make_float2(-m_used, -m_used);
+            float2 sum2 = make_float2(0.f, 0.f);
 #pragma unroll
-            for (int c = 0; c < 2; ++c) {
-                uint32_t pk[32];
+            for (int q = 0; q < 4; ++q) {
+                uint32_t x[32];
+                tmem_ld32(tS + q * 32, x);
+                tmem_wait_ld();
+                if (masked) {
 #pragma unroll
-                for (int j = 0; j < 32; ++j) {
-                    const int col = c * 64 + 2 * j;
-                    const float p0 = fast_exp2(fmaf(__uint_as_float(x[col >> 5][col & 31]),
-                                                    p.scale_log2, -m_used));
-                    const float p1 = fast_exp2(fmaf(__uint_as_float(x[(col + 1) >> 5][(col + 1) & 31]),
-                                                    p.scale_log2, -m_used));
-                    sum += p0 + p1;
-                    pk[j] = pack_bf16(p0, p1);
+                    for (int j = 0; j < 32; ++j)
+                        if (q * 32 + j >= limit) x[j] = 0xf149f2cau;
                 }
-                tmem_st32(tS + c * 32, pk);
+                uint32_t pk[16];
+#pragma unroll
+                for (int j = 0; j < 16; ++j) {
+                    const float2 a = __ffma2_rn(make_float2(__uint_as_float(x[2 * j]),
+                                                            __uint_as_float(x[2 * j + 1])), c2, nm2);
+                    float2 e;
+                    if (j % 3 == 2) {   // 5 pairs in 16 on the FMA pipe, the rest on MUFU
+                        e = exp2_poly2(a);
+                    } else {
+                        e.x = fast_exp2(a.x);
+                        e.y = fast_exp2(a.y);
+                    }
+                    sum2 = __fadd2_rn(sum2, e);
+                    pk[j] = pack_bf16(e.x, e.y);
+                }
+                tmem_st16(tS + q * 16, pk);
+                if (q & 1) {   // a half (64 keys) of P is complete: hand it to the MMA warp
+                    tmem_wait_st();
+                    tc_fence_before();
+                    mbar_arrive(&bar_P[2 * s + (q >> 1)]);
+                }
             }
-            l += sum;
-            tmem_wait_st();
-            tc_fence_before();
-            mbar_arrive(&bar_P[s]);
+            l += sum2.x + sum2.y;
         }
         if (n_iter > 0) {
             mbar_wait(bar_done, 0);
             tc_fence_after();
             const float inv = 1.f / l;
-            const bool valid = t < p.Lq;
-            __nv_bfloat16* orow = p.O + int64_t(t) * p.o_stride_tok + int64_t(h) * p.o_stride_head;
+            const bool valid = t < Ls;
+            __nv_bfloat16* orow = p.O + int64_t(tok0 + t) * p.o_stride_tok + int64_t(h) * p.o_stride_head;
 #pragma unroll
-            for (int c = 0; c < D / 32; ++c) {
+            for (int q = 0; q < D / 32; ++q) {
                 uint32_t o[32];
-                tmem_ld32(tO + c * 32, o);
+                tmem_ld32(tO + q * 32, o);
                 tmem_wait_ld();
                 if (valid) {
 #pragma unroll
@@ -291,12 +344,12 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                         v.y = pack_bf16(__uint_as_float(o[j + 2]) * inv, __uint_as_float(o[j + 3]) * inv);
                         v.z = pack_bf16(__uint_as_float(o[j + 4]) * inv, __uint_as_float(o[j + 5]) * inv);
                         v.w = pack_bf16(__uint_as_float(o[j + 6]) * inv, __uint_as_float(o[j + 7]) * inv);
-                        *reinterpret_cast<uint4*>(orow + c * 32 + j) = v;
+                        *reinterpret_cast<uint4*>(orow + q * 32 + j) = v;
                     }
                 }
             }
             if (valid)
-                p.LSE[int64_t(h) * p.lse_stride + t] = (m_used + log2f(l)) * 0.6931471805599453f;
+                p.LSE[int64_t(h) * p.lse_stride + tok0 + t] = (m_used + log2f(l)) * 0.6931471805599453f;
         }
     }
     tc_fence_before();

@@ -225,18 +225,35 @@ pf_status set_attrs() {
     return PF_OK;
 }
 
-// ---- forward launch: queries [Lq] attend to prefix source [Lp] (all visible) + own causal keys
+// Sequence table of one launch from host offsets cu[0..n] (cu[0] = 0, n <= kMaxSeqs)
+pf::SeqTable make_seq_table(int n, const int64_t* cu) {
+    pf::SeqTable t;
+    memset(&t, 0, sizeof(t));
+    t.n = n;
+    for (int s = 0; s <= n; ++s) t.cu[s] = int(cu[s]);
+    for (int s = 0; s < n; ++s) {
+        const int Ls = t.cu[s + 1] - t.cu[s];
+        t.pqs[s + 1] = t.pqs[s] + (Ls + 63) / 64;
+        t.ckt[s + 1] = t.ckt[s] + (Ls + 127) / 128;
+    }
+    return t;
+}
+
+// ---- forward launch over n sequences packed along the token axis: the queries of sequence s
+// attend to the prefix source [Lp] (all visible) + the keys of s causally
 template <int D>
 pf_status launch_fwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const pf_tensor& V1,
                      int64_t Lp, const pf_tensor& K2, const pf_tensor& V2, const pf_tensor& O,
-                     float* LSE, int64_t lse_stride, int64_t Lq, int prof_kind, cudaStream_t s) {
+                     float* LSE, int64_t lse_stride, int n, const int64_t* cu, int prof_kind,
+                     cudaStream_t s) {
     pf_ctx* ctx = g->ctx;
     const int Hq = g->desc.n_q_heads, Hkv = g->desc.n_kv_heads;
+    const int64_t total = cu[n];
     CUtensorMap mQ, mK1, mV1, mK2, mV2;
     pf_status st;
-    if ((st = make_map(ctx, &mQ, "Q", Q, Lq, Hq, D))) return st;
-    if ((st = make_map(ctx, &mK2, "K", K2, Lq, Hkv, D))) return st;
-    if ((st = make_map(ctx, &mV2, "V", V2, Lq, Hkv, D))) return st;
+    if ((st = make_map(ctx, &mQ, "Q", Q, total, Hq, D))) return st;
+    if ((st = make_map(ctx, &mK2, "K", K2, total, Hkv, D))) return st;
+    if ((st = make_map(ctx, &mV2, "V", V2, total, Hkv, D))) return st;
     if (Lp > 0) {
         if ((st = make_map(ctx, &mK1, "K1", K1, Lp, Hkv, D))) return st;
         if ((st = make_map(ctx, &mV1, "V1", V1, Lp, Hkv, D))) return st;
@@ -250,15 +267,16 @@ pf_status launch_fwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const
     p.o_stride_head = O.stride_head;
     p.LSE = LSE;
     p.lse_stride = lse_stride;
-    p.Lq = int(Lq);
     p.Lp = int(Lp);
     p.Hq = Hq;
     p.Hkv = Hkv;
     p.G = Hq / Hkv;
-    p.nRB = int((Lq + 127) / 128);
     p.scale_log2 = g->sigma * 1.4426950408889634f;
-    const int nItems = p.nRB * p.G;
-    dim3 grid((nItems + 1) / 2, Hkv);
+    p.seq = make_seq_table(n, cu);
+    int ctas = 0;
+    for (int i = 0; i < n; ++i) ctas += ((p.seq.ckt[i + 1] - p.seq.ckt[i]) * p.G + 1) / 2;
+    if (ctas == 0) return PF_OK;
+    dim3 grid(ctas, Hkv);
     {
         ProfScope prof(ctx, prof_kind, s);
         pf::attn_fwd_kernel<D><<<grid, pf::FwdCfg<D>::THREADS, pf::FwdCfg<D>::SMEM, s>>>(
@@ -267,20 +285,6 @@ pf_status launch_fwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const
     PF_CUDA(ctx, cudaGetLastError());
     ctx->n_launches += 1;
     return PF_OK;
-}
-
-// Sequence table of one backward launch from host offsets cu[0..n] (cu[0] = 0, n <= kMaxSeqs)
-pf::SeqTable make_seq_table(int n, const int64_t* cu) {
-    pf::SeqTable t;
-    memset(&t, 0, sizeof(t));
-    t.n = n;
-    for (int s = 0; s <= n; ++s) t.cu[s] = int(cu[s]);
-    for (int s = 0; s < n; ++s) {
-        const int Ls = t.cu[s + 1] - t.cu[s];
-        t.pqs[s + 1] = t.pqs[s] + (Ls + 63) / 64;
-        t.ckt[s + 1] = t.ckt[s] + (Ls + 127) / 128;
-    }
-    return t;
 }
 
 // ---- backward launch over a wave of n sequences packed along the token axis.  Keys of the prefix
@@ -594,8 +598,9 @@ pf_status pf_phaseA_fwd(pf_group* grp, pf_tensor Q1, pf_tensor O1, float* LSE1, 
     if (Lp > 0) {
         cudaStream_t s = static_cast<cudaStream_t>(stream);
         pf_tensor none = {nullptr, 0, 0};
-        st = d == 64 ? launch_fwd<64>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, Lp, 0, s)
-                     : launch_fwd<128>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, Lp, 0, s);
+        const int64_t cu[2] = {0, Lp};
+        st = d == 64 ? launch_fwd<64>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, 1, cu, 0, s)
+                     : launch_fwd<128>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, 1, cu, 0, s);
         if (st) return st;
     }
     grp->state = 1;
@@ -619,13 +624,22 @@ pf_status pf_phaseB_fwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens
     if ((st = check_tensor(ctx, "O2", O2, total, Hq, d))) return st;
     if (total > 0 && !LSE2) return fail(ctx, PF_INVALID_ARG, "LSE2 is NULL");
     cudaStream_t s = static_cast<cudaStream_t>(stream);
-    for (int i = 0; i < n_seqs; ++i) {
-        const int64_t t0 = cu_seqlens_host[i], Ls = cu_seqlens_host[i + 1] - t0;
-        if (Ls == 0) continue;
+    int i = 0;
+    while (i < n_seqs) {   // launches of <= kMaxSeqs non-empty sequences
+        int64_t cu[pf::kMaxSeqs + 1];
+        int n = 0;
+        int64_t t0 = 0;
+        for (; i < n_seqs && n < pf::kMaxSeqs; ++i) {
+            const int64_t b = cu_seqlens_host[i], Ls = cu_seqlens_host[i + 1] - b;
+            if (Ls == 0) continue;
+            if (n == 0) { t0 = b; cu[0] = 0; }
+            cu[++n] = b + Ls - t0;
+        }
+        if (n == 0) break;
         const pf_tensor q = tok_offset(Q2, t0), k = tok_offset(K2, t0), v = tok_offset(V2, t0),
                         o = tok_offset(O2, t0);
-        st = d == 64 ? launch_fwd<64>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, Ls, 1, s)
-                     : launch_fwd<128>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, Ls, 1, s);
+        st = d == 64 ? launch_fwd<64>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, n, cu, 1, s)
+                     : launch_fwd<128>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, n, cu, 1, s);
         if (st) return st;
     }
     return PF_OK;
