@@ -23,6 +23,11 @@
 #include "sm100_ptx.cuh"
 #include "seq_table.cuh"
 
+// exp2 evaluations (per 16 pairs) done by the polynomial on the FMA pipe instead of MUFU.EX2
+#ifndef PF_FWD_POLY16
+#define PF_FWD_POLY16 5
+#endif
+
 namespace pf {
 
 struct FwdParams {
@@ -254,21 +259,27 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             const bool masked = limit < 128;     // ragged prefix tail or causal diagonal
             // ---- pass 1: row maximum (S is read from TMEM twice to keep the live registers low)
             float mx0 = -INFINITY, mx1 = -INFINITY;
-#pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                uint32_t x[32];
-                tmem_ld32(tS + q * 32, x);
+            {
+                uint32_t x[4][32];
+                tmem_ld32(tS + 0, x[0]);
+                tmem_ld32(tS + 32, x[1]);
+                tmem_ld32(tS + 64, x[2]);
+                tmem_ld32(tS + 96, x[3]);
                 tmem_wait_ld();
                 if (masked) {
 #pragma unroll
-                    for (int j = 0; j < 32; ++j)
-                        if (q * 32 + j >= limit) x[j] = 0xf149f2cau;  // -1e30: exp2 -> 0, stays finite
+                    for (int q = 0; q < 4; ++q)
+#pragma unroll
+                        for (int j = 0; j < 32; ++j)
+                            if (q * 32 + j >= limit) x[q][j] = 0xf149f2cau;  // -1e30: exp2 -> 0, stays finite
                 }
 #pragma unroll
-                for (int j = 0; j < 32; j += 2) {
-                    mx0 = fmaxf(mx0, __uint_as_float(x[j]));
-                    mx1 = fmaxf(mx1, __uint_as_float(x[j + 1]));
-                }
+                for (int q = 0; q < 4; ++q)
+#pragma unroll
+                    for (int j = 0; j < 32; j += 2) {
+                        mx0 = fmaxf(mx0, __uint_as_float(x[q][j]));
+                        mx1 = fmaxf(mx1, __uint_as_float(x[q][j + 1]));
+                    }
             }
             const float m_new = fmaxf(mx0, mx1) * c;
             // lazy rescale: keep a stale max while the new one is within 2^8 of it
@@ -291,11 +302,13 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             // (S columns [32q, 32q+32)) writes P columns [16q, 16q+16): always behind the reads.
             const float2 c2 = make_float2(c, c), nm2 = make_float2(-m_used, -m_used);
             float2 sum2 = make_float2(0.f, 0.f);
+            uint32_t xb[2][32];                  // chunk q+1 is in flight while chunk q is exponentiated
+            tmem_ld32(tS, xb[0]);
+            tmem_wait_ld();
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
-                uint32_t x[32];
-                tmem_ld32(tS + q * 32, x);
-                tmem_wait_ld();
+                uint32_t (&x)[32] = xb[q & 1];
+                if (q < 3) tmem_ld32(tS + (q + 1) * 32, xb[(q + 1) & 1]);
                 if (masked) {
 #pragma unroll
                     for (int j = 0; j < 32; ++j)
@@ -307,7 +320,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     const float2 a = __ffma2_rn(make_float2(__uint_as_float(x[2 * j]),
                                                             __uint_as_float(x[2 * j + 1])), c2, nm2);
                     float2 e;
-                    if (j % 3 == 2) {   // 5 pairs in 16 on the FMA pipe, the rest on MUFU
+                    if ((j * PF_FWD_POLY16) % 16 < PF_FWD_POLY16) {   // PF_FWD_POLY16 pairs in 16 on the FMA pipe
                         e = exp2_poly2(a);
                     } else {
                         e.x = fast_exp2(a.x);
@@ -316,6 +329,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     sum2 = __fadd2_rn(sum2, e);
                     pk[j] = pack_bf16(e.x, e.y);
                 }
+                tmem_wait_ld();                  // chunk q+1 landed (and every read of columns < 32(q+2) is done)
                 tmem_st16(tS + q * 16, pk);
                 if (q & 1) {   // a half (64 keys) of P is complete: hand it to the MMA warp
                     tmem_wait_st();
