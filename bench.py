@@ -243,8 +243,10 @@ def main() -> None:
     ap.add_argument("--cpu-budget", type=float, default=6e11, help="algorithmic flops of the oracle sample")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--wave", type=int, default=1,
-                    help="suffixes packed per Phase-B call (PAPER.md:158 suffix microbatch); 0 = all N")
+    ap.add_argument("--wave", type=int, default=0,
+                    help="suffixes packed per Phase-B call (PAPER.md:158, 242 suffix microbatch); "
+                         "0 = all N in one wave (default), 1 = one call per suffix")
+    ap.add_argument("--no-wave1", action="store_true", help="skip the extra wave = 1 measurement")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -258,6 +260,7 @@ def main() -> None:
     import torch
     import torch.distributed as dist
     from paper_2606_01143_b200 import binding as pf          # raises if libprefixflow.so is missing
+    from paper_2606_01143_b200 import dist as pfd
     from paper_2606_01143_b200 import inputs, schedule
 
     if not torch.cuda.is_available():
@@ -270,8 +273,7 @@ def main() -> None:
 
     shape = pick_config(args.config)
     # weak scaling over independent rollout groups: rank r draws its own group
-    if world > 1:
-        shape.seed += 100000 * rank
+    shape = pfd.rank_shape(shape, rank)
     F = flops(shape)
     peaks = measured_peaks()
     ctx = pf.pf_create(local_rank)
@@ -295,12 +297,7 @@ def main() -> None:
             fn()
         e1.record(stream)
         barrier()
-        ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
-        return ms / steps
+        return pfd.max_over_ranks(e0.elapsed_time(e1), dev) / steps
 
     step = lambda: schedule.run_prefixflow_step(ctx, g, stream)
     torch.cuda.reset_peak_memory_stats()
@@ -362,11 +359,37 @@ def main() -> None:
         del r
         torch.cuda.empty_cache()
 
+    # ---- the same step with one Phase-B call per suffix (the paper's "separate" organisation) ----
+    wave1 = None
+    if wave != 1 and not args.no_wave1:
+        g1 = schedule.to_device(inp, dev, wave=1)
+        step1 = lambda: schedule.run_prefixflow_step(ctx, g1, stream)
+        for _ in range(args.warmup):
+            step1()
+        ms1 = timed(step1, args.steps)
+        pf.pf_set_option(ctx, "profile", 1)
+        for k in range(4):
+            pf.pf_profile_read(ctx, k)
+        timed(step1, args.steps)
+        p1 = {name: pf.pf_profile_read(ctx, k) for k, name in enumerate(["A_fwd", "B_fwd", "B_bwd", "C_bwd"])}
+        pf.pf_set_option(ctx, "profile", 0)
+        bf_ms, bb_ms = p1["B_fwd"][1] / steps, p1["B_bwd"][1] / steps
+        wave1 = dict(ms_per_step=ms1, tflops=world * F["step"] / (ms1 * 1e-3) / 1e12,
+                     B_fwd=dict(ms=bf_ms, tflops=tf(F["B_fwd"], bf_ms), launches_per_step=p1["B_fwd"][0] // steps),
+                     B_bwd=dict(ms=bb_ms, tflops=tf(F["B_bwd"], bb_ms), launches_per_step=p1["B_bwd"][0] // steps),
+                     phaseB_tflops=tf(F["B_fwd"] + F["B_bwd"], bf_ms + bb_ms),
+                     phaseB_pct_of_bf16_burst=100 * tf(F["B_fwd"] + F["B_bwd"], bf_ms + bb_ms) / peaks["burst"],
+                     speedup_vs_replay=(replay["ms_per_step"] / ms1) if replay else None)
+        del g1
+        torch.cuda.empty_cache()
+
     # ---- end to end: pinned host inputs -> device, step, results -> pinned host, every step ----
     e2e = None
     if not args.no_e2e:
-        ins = [g.Q1, g.K1, g.V1, g.dO1] + g.Q2 + g.K2 + g.V2 + g.dO2
-        outs = [g.O1, g.LSE1, g.dQ1, g.dK1, g.dV1, g.gK1, g.gV1] + g.O2 + g.LSE2 + g.dQ2 + g.dK2 + g.dV2
+        pk = g.packed   # the packed wave tensors (the per-suffix entries of g.Q2 ... are views of them)
+        ins = [g.Q1, g.K1, g.V1, g.dO1] + [w[k] for w in pk for k in ("Q2", "K2", "V2", "dO2")]
+        outs = [g.O1, g.LSE1, g.dQ1, g.dK1, g.dV1, g.gK1, g.gV1] + \
+               [w[k] for w in pk for k in ("O2", "LSE2", "dQ2", "dK2", "dV2")]
         h_in = [torch.empty(t.shape, dtype=t.dtype, pin_memory=True).copy_(t) for t in ins]
         h_out = [torch.empty(t.shape, dtype=t.dtype, pin_memory=True) for t in outs]
         bi = sum(t.numel() * t.element_size() for t in ins)
@@ -413,7 +436,7 @@ def main() -> None:
                                    pct_of_bf16_sustained=100 * phaseB_tflops / peaks["sustained"] if phaseB_tflops else None,
                                    pct_of_bf16_nominal=100 * phaseB_tflops / 2250.0 if phaseB_tflops else None),
         ms_per_step_profiled=ms_step_prof, non_attention_ms=other_ms,
-        replay=replay, flops=dict(A=F["A"], B_fwd=F["B_fwd"], B_bwd=F["B_bwd"], C=F["C"], step=F["step"],
+        replay=replay, wave1=wave1, flops=dict(A=F["A"], B_fwd=F["B_fwd"], B_bwd=F["B_bwd"], C=F["C"], step=F["step"],
                                   replay=F["replay"]),
         peak_hbm_bytes=peak_hbm, peaks=peaks)
     pf.pf_destroy(ctx)

@@ -149,11 +149,14 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     const bool pre = item < p.nItemsP;
     int kt, g, pair_lo, pair_hi, qs_lo, kvrow0;
     if (pre) {
-        const int per = p.Hkv * p.chunksP;
-        kt = item / per;
+        // chunk-major order: the CTAs that run at the same time walk the SAME (sequence, head) pairs
+        // over different key tiles, so their Q/dO tiles and the dQ^T tiles they reduce into stay
+        // L2-resident instead of streaming the whole fp32 dQ workspace through HBM
+        const int per = p.nPT * p.Hkv;
         const int r = item % per;
-        g = r / p.chunksP;
-        pair_lo = (r % p.chunksP) * p.ppcP;
+        kt = r / p.Hkv;
+        g = r % p.Hkv;
+        pair_lo = (item / per) * p.ppcP;
         pair_hi = min(p.seq.n * p.G, pair_lo + p.ppcP);
         qs_lo = 0;
         kvrow0 = kt * 128;
