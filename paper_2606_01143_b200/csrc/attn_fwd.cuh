@@ -9,13 +9,14 @@
 //
 // One CTA = two query tiles of 128 rows ("slots": consecutive (row block, q head) items of one KV
 // head and one sequence, so both read the same K/V stream) ping-ponged on the tensor core:
-//   warps 0-3  softmax of slot 0   (thread r <-> query row r <-> TMEM lane r)
-//   warps 4-7  softmax of slot 1
-//   warp  8    TMA producer (Q once, K/V tiles through a 2-stage ring)
-//   warp  9    tcgen05.mma issuer (one thread)
-// TMEM (512 columns): S0 | S1 | O0 | O1, 128 fp32 columns each; P (bf16) overwrites the first 64
-// columns of its S and is consumed from TMEM as the A operand of P.V, handed over in two halves
-// (keys 0-63, 64-127) so that P.V starts while the second half is still being exponentiated.
+//   warps 0-7   softmax of slot 0: warps 0-3 key columns [0,64), warps 4-7 key columns [64,128)
+//   warps 8-15  softmax of slot 1   (thread r of a warpgroup <-> query row r <-> TMEM lane r)
+//   warp  16    TMA producer (Q once, K/V tiles through a 2-stage ring)
+//   warp  17    tcgen05.mma issuer (one thread)
+// TMEM (512 columns): S0 | S1 | O0 | O1, 128 fp32 columns each; each column half of P (bf16, 32
+// columns) overwrites the start of its own half of S and is consumed from TMEM as the A operand of
+// P.V; the two halves are handed over separately.  The two warpgroups of a slot exchange their
+// partial row maxima through shared memory once per KV tile.
 // A quarter of the exponentials is evaluated by a degree-3 polynomial on the FMA pipe, the rest by
 // MUFU.EX2 (16 / clk / SM, which alone would tie with the tensor pipe).
 #pragma once
@@ -51,8 +52,9 @@ struct FwdCfg {
     static constexpr int OFF_K = 2 * TILE;             // KS tiles
     static constexpr int OFF_V = OFF_K + KS * TILE;    // KS tiles
     static constexpr int OFF_BAR = OFF_V + KS * TILE;
-    static constexpr int SMEM = OFF_BAR + 256;
-    static constexpr int THREADS = 320;
+    static constexpr int OFF_X = OFF_BAR + 256;        // row-max / row-sum exchange between column halves
+    static constexpr int SMEM = OFF_X + 2 * 2 * 2 * 128 * 4;
+    static constexpr int THREADS = 576;
 };
 
 // 2^x for a pair of x <= ~8 on the FMA / ALU pipes (packed f32x2 math): round-to-nearest split
@@ -74,7 +76,7 @@ __device__ __forceinline__ float2 exp2_poly2(float2 x) {
 }
 
 template <int D>
-__global__ void __launch_bounds__(320, 1)
+__global__ void __launch_bounds__(576, 1)
 attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK1,
                 const __grid_constant__ CUtensorMap tmV1, const __grid_constant__ CUtensorMap tmK2,
                 const __grid_constant__ CUtensorMap tmV2, const __grid_constant__ FwdParams p) {
@@ -125,7 +127,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         mbar_init(bar_done, 1);
         fence_mbar_init();
     }
-    if (warp == 8) {
+    if (warp == 16) {
         tmem_alloc(tmem_slot, 512);
         if (elect_one()) {
             tma_prefetch_desc(&tmQ); tma_prefetch_desc(&tmK1); tma_prefetch_desc(&tmV1);
@@ -137,7 +139,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
 
-    if (warp == 8) {
+    if (warp == 16) {
         // =============================== TMA producer ===============================
         if (elect_one()) {
             mbar_arrive_expect_tx(&bar_Q[0], C::TILE);
@@ -166,7 +168,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                                 &bar_Vf[st], 64 * k, g, row0);
             }
         }
-    } else if (warp == 9) {
+    } else if (warp == 17) {
         // =============================== MMA issuer ===============================
         if (elect_one()) {
             constexpr uint32_t idesc_qk = make_idesc_bf16(128, 128, false, false);
@@ -186,7 +188,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 const uint64_t v = make_smem_desc_sw128(sV + st * C::TILE, C::SUB, 1024);
 #pragma unroll
                 for (int kk = half * 4; kk < half * 4 + 4; ++kk)
-                    mma_ts(tmem + 256 + s * D, tmem + s * 128 + kk * 8, v + ((kk * 2048) >> 4), idesc_pv,
+                    mma_ts(tmem + 256 + s * D, tmem + s * 128 + half * 64 + (kk & 3) * 8, v + ((kk * 2048) >> 4), idesc_pv,
                            (acc || kk > 0) ? 1u : 0u);
             };
             mbar_wait(&bar_Q[0], 0);
@@ -241,54 +243,59 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         }
     } else {
         // =============================== softmax warpgroups ===============================
-        const int s = warp >> 2;                 // slot
+        const int s = warp >> 3;                 // slot
+        const int hh = (warp >> 2) & 1;          // key-column half of the S tile
         const int r = tid & 127;                 // row in tile == TMEM lane
         const int n_iter = s == 0 ? n_iter0 : n_iter1;
         const int rb = s == 0 ? rb0 : rb1;
         const int h = s == 0 ? h0 : h1;
         const int t = rb * 128 + r;              // query row within its sequence
         const uint32_t lane_off = uint32_t((warp & 3) * 32) << 16;
-        const uint32_t tS = tmem + s * 128 + lane_off;
-        const uint32_t tO = tmem + 256 + s * D + lane_off;
+        const uint32_t tS = tmem + s * 128 + hh * 64 + lane_off;       // this half of S; P at its start
+        const uint32_t tO = tmem + 256 + s * D + hh * (D / 2) + lane_off;  // this half of the O columns
+        float* xch = reinterpret_cast<float*>(smem + C::OFF_X) + s * 256;  // [parity][slot][half][128]
         const float c = p.scale_log2;
         float m_used = -INFINITY, l = 0.f;
         for (int it = 0; it < n_iter; ++it) {
             mbar_wait(&bar_S[s], it & 1);
             tc_fence_after();
-            const int limit = it < nP ? p.Lp - it * 128 : t - (it - nP) * 128 + 1;
-            const bool masked = limit < 128;     // ragged prefix tail or causal diagonal
+            // visible keys of this tile for this row, relative to this half's first column
+            const int limit = (it < nP ? p.Lp - it * 128 : t - (it - nP) * 128 + 1) - hh * 64;
+            const bool masked = limit < 64;      // ragged prefix tail or causal diagonal
             // ---- pass 1: row maximum (S is read from TMEM twice to keep the live registers low)
             float mx0 = -INFINITY, mx1 = -INFINITY;
             {
-                uint32_t x[4][32];
+                uint32_t x[2][32];
                 tmem_ld32(tS + 0, x[0]);
                 tmem_ld32(tS + 32, x[1]);
-                tmem_ld32(tS + 64, x[2]);
-                tmem_ld32(tS + 96, x[3]);
                 tmem_wait_ld();
                 if (masked) {
 #pragma unroll
-                    for (int q = 0; q < 4; ++q)
+                    for (int q = 0; q < 2; ++q)
 #pragma unroll
                         for (int j = 0; j < 32; ++j)
                             if (q * 32 + j >= limit) x[q][j] = 0xf149f2cau;  // -1e30: exp2 -> 0, stays finite
                 }
 #pragma unroll
-                for (int q = 0; q < 4; ++q)
+                for (int q = 0; q < 2; ++q)
 #pragma unroll
                     for (int j = 0; j < 32; j += 2) {
                         mx0 = fmaxf(mx0, __uint_as_float(x[q][j]));
                         mx1 = fmaxf(mx1, __uint_as_float(x[q][j + 1]));
                     }
             }
-            const float m_new = fmaxf(mx0, mx1) * c;
+            float* xm = xch + (it & 1) * 512;
+            const float mine = fmaxf(mx0, mx1);
+            xm[hh * 128 + r] = mine;
+            named_bar_sync(1 + s, 256);          // the two warpgroups of the slot
+            const float m_new = fmaxf(mine, xm[(hh ^ 1) * 128 + r]) * c;
             // lazy rescale: keep a stale max while the new one is within 2^8 of it
             const bool need = (it == 0) || (m_new > m_used + 8.f);
             if (__any_sync(0xffffffffu, need && it > 0)) {
                 const float alpha = need ? fast_exp2(m_used - m_new) : 1.f;
                 l *= alpha;
 #pragma unroll
-                for (int q = 0; q < D / 32; ++q) {
+                for (int q = 0; q < D / 64; ++q) {
                     uint32_t o[32];
                     tmem_ld32(tO + q * 32, o);
                     tmem_wait_ld();
@@ -298,17 +305,17 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 }
             }
             if (need) m_used = m_new;
-            // ---- pass 2: P = exp2(c S - m), packed to bf16 over the first 64 columns of S.  Chunk q
-            // (S columns [32q, 32q+32)) writes P columns [16q, 16q+16): always behind the reads.
+            // ---- pass 2: P = exp2(c S - m), packed to bf16 over the first 32 columns of this half
+            // of S.  Chunk q (columns [32q, 32q+32)) writes P columns [16q, 16q+16): behind the reads.
             const float2 c2 = make_float2(c, c), nm2 = make_float2(-m_used, -m_used);
             float2 sum2 = make_float2(0.f, 0.f);
-            uint32_t xb[2][32];                  // chunk q+1 is in flight while chunk q is exponentiated
+            uint32_t xb[2][32];                  // chunk 1 is in flight while chunk 0 is exponentiated
             tmem_ld32(tS, xb[0]);
             tmem_wait_ld();
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-                uint32_t (&x)[32] = xb[q & 1];
-                if (q < 3) tmem_ld32(tS + (q + 1) * 32, xb[(q + 1) & 1]);
+            for (int q = 0; q < 2; ++q) {
+                uint32_t (&x)[32] = xb[q];
+                if (q == 0) tmem_ld32(tS + 32, xb[1]);
                 if (masked) {
 #pragma unroll
                     for (int j = 0; j < 32; ++j)
@@ -329,24 +336,28 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     sum2 = __fadd2_rn(sum2, e);
                     pk[j] = pack_bf16(e.x, e.y);
                 }
-                tmem_wait_ld();                  // chunk q+1 landed (and every read of columns < 32(q+2) is done)
+                tmem_wait_ld();
                 tmem_st16(tS + q * 16, pk);
-                if (q & 1) {   // a half (64 keys) of P is complete: hand it to the MMA warp
-                    tmem_wait_st();
-                    tc_fence_before();
-                    mbar_arrive(&bar_P[2 * s + (q >> 1)]);
-                }
             }
+            tmem_wait_st();
+            tc_fence_before();
+            mbar_arrive(&bar_P[2 * s + hh]);     // this half (64 keys) of P is ready for the MMA warp
             l += sum2.x + sum2.y;
         }
         if (n_iter > 0) {
+            // combine the two halves' row sums, then each half normalises its half of the O columns
+            float* xl = xch + (n_iter & 1) * 512;
+            xl[hh * 128 + r] = l;
+            named_bar_sync(1 + s, 256);
+            l += xl[(hh ^ 1) * 128 + r];
             mbar_wait(bar_done, 0);
             tc_fence_after();
             const float inv = 1.f / l;
             const bool valid = t < Ls;
-            __nv_bfloat16* orow = p.O + int64_t(tok0 + t) * p.o_stride_tok + int64_t(h) * p.o_stride_head;
+            __nv_bfloat16* orow = p.O + int64_t(tok0 + t) * p.o_stride_tok + int64_t(h) * p.o_stride_head +
+                                  hh * (D / 2);
 #pragma unroll
-            for (int q = 0; q < D / 32; ++q) {
+            for (int q = 0; q < D / 64; ++q) {
                 uint32_t o[32];
                 tmem_ld32(tO + q * 32, o);
                 tmem_wait_ld();
@@ -362,13 +373,13 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     }
                 }
             }
-            if (valid)
+            if (valid && hh == 0)
                 p.LSE[int64_t(h) * p.lse_stride + tok0 + t] = (m_used + log2f(l)) * 0.6931471805599453f;
         }
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 8) tmem_dealloc(tmem, 512);
+    if (warp == 16) tmem_dealloc(tmem, 512);
 }
 
 }  // namespace pf
