@@ -360,8 +360,9 @@ pf_status launch_bwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const
                                            : int(std::lround(target / std::fmax(1.0, avg_nqs)));
     ppcP = ppcP < 1 ? 1 : (ppcP > pairs ? pairs : ppcP);
     int ppcC = ctx->bwd_heads_per_item > 0 ? ctx->bwd_heads_per_item
-                                           : int(std::lround(target / std::fmax(1.0, avg_nqs / 2)));
-    ppcC = ppcC < 1 ? 1 : (ppcC > G ? G : ppcC);
+                                           : int(std::lround(target / std::fmax(1.0, avg_nqs)));
+    const int capC = ctx->bwd_heads_per_item > 0 ? G : (G + 1) / 2;   // measured: G heads per causal item is too coarse
+    ppcC = ppcC < 1 ? 1 : (ppcC > capC ? capC : ppcC);
     p.ppcP = ppcP; p.chunksP = (pairs + ppcP - 1) / ppcP;
     p.ppcC = ppcC; p.chunksC = (G + ppcC - 1) / ppcC;
     p.nItemsP = p.nPT * Hkv * p.chunksP;
