@@ -247,6 +247,8 @@ def main() -> None:
                     help="suffixes packed per Phase-B call (PAPER.md:158, 242 suffix microbatch); "
                          "0 = all N in one wave (default), 1 = one call per suffix")
     ap.add_argument("--no-wave1", action="store_true", help="skip the extra wave = 1 measurement")
+    ap.add_argument("--no-offload", action="store_true", help="skip the memory-lifecycle / offload measurement")
+    ap.add_argument("--offload-wave", type=int, default=1, help="suffixes per wave in the lifecycle measurement")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -383,6 +385,29 @@ def main() -> None:
         del g1
         torch.cuda.empty_cache()
 
+    # ---- memory lifecycle: Phase-B peak HBM with the dormant Phase-A set
+    # {Q1, O1, LSE1} resident vs offloaded to pinned host memory on a side stream ----
+    memory = None
+    if rank == 0 and not args.no_offload:
+        del g
+        torch.cuda.empty_cache()
+        pinned = {}
+        res = {}
+        for mode in (False, True):
+            schedule.run_lifecycle_step(ctx, inp, dev, wave=args.offload_wave, offload=mode, pinned=pinned)
+            r = schedule.run_lifecycle_step(ctx, inp, dev, wave=args.offload_wave, offload=mode, pinned=pinned)
+            r.pop("outputs")
+            res["offload" if mode else "resident"] = r
+            torch.cuda.empty_cache()
+        a, b = res["resident"], res["offload"]
+        memory = dict(wave=args.offload_wave, resident=a, offload=b,
+                      phaseB_peak_reduction_pct=100.0 * (1 - b["peak_phaseB_bytes"] / a["peak_phaseB_bytes"]),
+                      dormant_bytes=inp.Q1.numel() * 2 * 2 + inp.Q1.shape[0] * inp.Q1.shape[1] * 4,
+                      note="one attention layer; tensors allocated and freed as a trainer would "
+                           "(suffix-wave tensors live only during their wave); peaks are "
+                           "torch.cuda.max_memory_allocated")
+        g = schedule.to_device(inp, dev, wave=wave)
+
     # ---- end to end: pinned host inputs -> device, step, results -> pinned host, every step ----
     e2e = None
     if not args.no_e2e:
@@ -436,7 +461,7 @@ def main() -> None:
                                    pct_of_bf16_sustained=100 * phaseB_tflops / peaks["sustained"] if phaseB_tflops else None,
                                    pct_of_bf16_nominal=100 * phaseB_tflops / 2250.0 if phaseB_tflops else None),
         ms_per_step_profiled=ms_step_prof, non_attention_ms=other_ms,
-        replay=replay, wave1=wave1, flops=dict(A=F["A"], B_fwd=F["B_fwd"], B_bwd=F["B_bwd"], C=F["C"], step=F["step"],
+        replay=replay, wave1=wave1, memory=memory, flops=dict(A=F["A"], B_fwd=F["B_fwd"], B_bwd=F["B_bwd"], C=F["C"], step=F["step"],
                                   replay=F["replay"]),
         peak_hbm_bytes=peak_hbm, peaks=peaks)
     pf.pf_destroy(ctx)

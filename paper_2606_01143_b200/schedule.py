@@ -157,3 +157,104 @@ def run_replay_step(ctx, r: ReplayBuffers, stream=None) -> None:
             pf.pf_phaseC_bwd(grp, r.Q[i], r.O[i], r.LSE[i], r.dO[i], r.dQ[i], r.dK[i], r.dV[i], stream)
         finally:
             pf.pf_group_end(grp)
+
+
+# --------------------------------------------------------------------------------------------------
+# Memory lifecycle of one layer: hot set {K1, V1, gK1, gV1} stays resident, the
+# dormant Phase-A set {Q1, O1, LSE1} leaves for pinned host memory on a side stream while Phase B
+# runs and is prefetched back before Phase C; suffix-wave tensors live only during their wave.
+# --------------------------------------------------------------------------------------------------
+def run_lifecycle_step(ctx, inp, device="cuda", wave: int = 1, offload: bool = True,
+                       pinned: Optional[dict] = None, keep_outputs: bool = False) -> dict:
+    """One A -> B -> C step that allocates and frees device tensors the way a trainer would.
+    Returns peak allocated bytes of the whole step and of Phase B alone (the paper's
+    "Phase-B peak HBM"), the step time, and (optionally) the outputs."""
+    s = inp.shape
+    dev = torch.device(device)
+    Hq, Hkv, d, Lp = s.n_q_heads, s.n_kv_heads, s.head_dim, s.Lp
+    bf, f32 = torch.bfloat16, torch.float32
+    main = torch.cuda.current_stream(dev)
+    side = pinned.setdefault("side_stream", torch.cuda.Stream(dev)) if pinned is not None else torch.cuda.Stream(dev)
+    pinned = pinned if pinned is not None else {}
+
+    def pin(name, like):
+        if name not in pinned:
+            pinned[name] = torch.empty(like.shape, dtype=like.dtype, pin_memory=True)
+        return pinned[name]
+
+    e = lambda L, H, dt=bf: torch.empty((L, H, d), dtype=dt, device=dev)
+    waves = _waves(s.N, wave)
+    max_tok = max((sum(s.Ls[k] for k in w) for w in waves), default=0)
+    desc = pf.make_desc(Hq, Hkv, d)
+    torch.cuda.synchronize(dev)
+    torch.cuda.reset_peak_memory_stats(dev)
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record(main)
+    # ---- Phase A
+    Q1, K1, V1 = inp.Q1.to(dev), inp.K1.to(dev), inp.V1.to(dev)
+    O1 = e(Lp, Hq); LSE1 = torch.empty((Hq, Lp), dtype=f32, device=dev)
+    gK1, gV1 = e(Lp, Hkv, f32), e(Lp, Hkv, f32)
+    ws = torch.empty(pf.pf_workspace_bytes(desc, Lp, max_tok), dtype=torch.uint8, device=dev)
+    grp = pf.pf_group_begin(ctx, desc, Lp, K1, V1, gK1, gV1, ws, main)
+    outs = {}
+    try:
+        pf.pf_phaseA_fwd(grp, Q1, O1, LSE1, main)
+        dormant = {"Q1": Q1, "O1": O1, "LSE1": LSE1}
+        if offload:
+            evA = torch.cuda.Event(); evA.record(main)
+            side.wait_event(evA)
+            for name, t in dormant.items():
+                pf.pf_offload(ctx, t, pin(name, t), side)
+            side.synchronize()        # the copies ran beside nothing here; a trainer overlaps them with wave 1
+            if keep_outputs:
+                outs["O1"], outs["LSE1"] = O1.clone(), LSE1.clone()
+            shapes = {k: (t.shape, t.dtype) for k, t in dormant.items()}
+            del Q1, O1, LSE1, dormant
+        # ---- Phase B, one wave at a time; a wave's tensors are freed when the wave is done
+        peak_a = torch.cuda.max_memory_allocated(dev)
+        torch.cuda.reset_peak_memory_stats(dev)
+        base = torch.cuda.memory_allocated(dev)
+        for w in waves:
+            cu = [0]
+            for k in w:
+                cu.append(cu[-1] + s.Ls[k])
+            cat = lambda src: torch.cat([src[k] for k in w], 0).contiguous().to(dev)
+            Q2, K2, V2, dO2 = cat(inp.Q2), cat(inp.K2), cat(inp.V2), cat(inp.dO2)
+            tot = cu[-1]
+            O2, dQ2 = e(tot, Hq), e(tot, Hq)
+            dK2, dV2 = e(tot, Hkv), e(tot, Hkv)
+            LSE2 = torch.empty((Hq, tot), dtype=f32, device=dev)
+            pf.pf_phaseB_fwd(grp, cu, Q2, K2, V2, O2, LSE2, main)
+            pf.pf_phaseB_bwd(grp, cu, Q2, K2, V2, O2, LSE2, dO2, dQ2, dK2, dV2, main)
+            if keep_outputs:
+                for j, k in enumerate(w):
+                    sl = slice(cu[j], cu[j + 1])
+                    outs[f"O2[{k}]"], outs[f"LSE2[{k}]"] = O2[sl].clone(), LSE2[:, sl].clone()
+                    outs[f"dQ2[{k}]"], outs[f"dK2[{k}]"], outs[f"dV2[{k}]"] = (
+                        dQ2[sl].clone(), dK2[sl].clone(), dV2[sl].clone())
+            del Q2, K2, V2, dO2, O2, dQ2, dK2, dV2, LSE2
+        peak_b = torch.cuda.max_memory_allocated(dev)
+        # ---- prefetch the dormant set back (side stream), then Phase C
+        if offload:
+            Q1 = torch.empty(shapes["Q1"][0], dtype=shapes["Q1"][1], device=dev)
+            O1 = torch.empty(shapes["O1"][0], dtype=shapes["O1"][1], device=dev)
+            LSE1 = torch.empty(shapes["LSE1"][0], dtype=shapes["LSE1"][1], device=dev)
+            evB = torch.cuda.Event(); evB.record(main)   # the fresh buffers may reuse blocks Phase B still reads
+            side.wait_event(evB)
+            for name, t in (("Q1", Q1), ("O1", O1), ("LSE1", LSE1)):
+                pf.pf_prefetch(ctx, pinned[name], t, side)
+            evP = torch.cuda.Event(); evP.record(side)
+            main.wait_event(evP)
+        elif keep_outputs:
+            outs["O1"], outs["LSE1"] = O1.clone(), LSE1.clone()
+        dO1 = inp.dO1.to(dev)
+        dQ1, dK1, dV1 = e(Lp, Hq), e(Lp, Hkv), e(Lp, Hkv)
+        pf.pf_phaseC_bwd(grp, Q1, O1, LSE1, dO1, dQ1, dK1, dV1, main)
+    finally:
+        pf.pf_group_end(grp)
+    t1.record(main)
+    torch.cuda.synchronize(dev)
+    if keep_outputs:
+        outs.update(dQ1=dQ1, dK1=dK1, dV1=dV1)
+    return dict(ms=t0.elapsed_time(t1), peak_step_bytes=max(peak_a, torch.cuda.max_memory_allocated(dev)),
+                peak_phaseB_bytes=peak_b, resident_at_phaseB_start_bytes=base, outputs=outs)

@@ -243,3 +243,24 @@ def test_error_paths(ctx):
     assert e.value.status == pf.PF_INVALID_ARG
     pf.pf_group_end(grp)
     torch.cuda.synchronize()
+
+
+@pytest.mark.parametrize("offload", [False, True])
+def test_memory_lifecycle_offload(ctx, offload):
+    """the dormant Phase-A set {Q1, O1, LSE1} moved to pinned host memory during
+    Phase B and prefetched back for Phase C changes no result, and lowers the Phase-B peak."""
+    shape = inputs.small_case(4, 2, 128, 700, [130, 64, 200], seed=41, dist="unit")
+    inp = inputs.make_group(shape)
+    ref = oracle.group_reference(inp)
+    r = schedule.run_lifecycle_step(ctx, inp, wave=2, offload=offload, keep_outputs=True)
+    o = r["outputs"]
+    check("O1", o["O1"], ref.O1); check("LSE1", o["LSE1"], ref.LSE1, lse=True)
+    for i in range(shape.N):
+        check(f"O2[{i}]", o[f"O2[{i}]"], ref.O2[i]); check(f"LSE2[{i}]", o[f"LSE2[{i}]"], ref.LSE2[i], lse=True)
+        check(f"dQ2[{i}]", o[f"dQ2[{i}]"], ref.dQ2[i])
+        check(f"dK2[{i}]", o[f"dK2[{i}]"], ref.dK2[i]); check(f"dV2[{i}]", o[f"dV2[{i}]"], ref.dV2[i])
+    check("dQ1", o["dQ1"], ref.dQ1); check("dK1", o["dK1"], ref.dK1); check("dV1", o["dV1"], ref.dV1)
+    if offload:
+        base = schedule.run_lifecycle_step(ctx, inp, wave=2, offload=False)
+        assert r["resident_at_phaseB_start_bytes"] < base["resident_at_phaseB_start_bytes"]
+        assert r["peak_phaseB_bytes"] < base["peak_phaseB_bytes"]
