@@ -7,18 +7,18 @@
 // visible to query t iff j <= t.  Phase A / replay: Lp = 0, one sequence.  Phase B: source 1 = the
 // cached prefix, the sequences are the suffixes of the wave packed along the token axis.
 //
-// One CTA = two query tiles of 128 rows ("slots": consecutive (row block, q head) items of one KV
-// head and one sequence, so both read the same K/V stream) ping-ponged on the tensor core:
-//   warps 0-7   softmax of slot 0: warps 0-3 key columns [0,64), warps 4-7 key columns [64,128)
-//   warps 8-15  softmax of slot 1   (thread r of a warpgroup <-> query row r <-> TMEM lane r)
-//   warp  16    TMA producer (Q once, K/V tiles through a 2-stage ring)
+// One CTA = one query tile of 128 rows of one head:
+//   warps 0-15  softmax: warpgroup q (warps 4q..4q+3) owns key columns [32q, 32q+32) of each S tile
+//               (thread r of a warpgroup <-> query row r <-> TMEM lane r)
+//   warp  16    TMA producer (K/V tiles through a 3-stage ring, prefix source then causal source)
 //   warp  17    tcgen05.mma issuer (one thread)
-// TMEM (512 columns): S0 | S1 | O0 | O1, 128 fp32 columns each; each column half of P (bf16, 32
-// columns) overwrites the start of its own half of S and is consumed from TMEM as the A operand of
-// P.V; the two halves are handed over separately.  The two warpgroups of a slot exchange their
-// partial row maxima through shared memory once per KV tile.
-// A quarter of the exponentials is evaluated by a degree-3 polynomial on the FMA pipe, the rest by
-// MUFU.EX2 (16 / clk / SM, which alone would tie with the tensor pipe).
+// TMEM: S[0] | S[1] | O | Q  (128 + 128 + D + D/2 columns).  Q (bf16) is written to TMEM once by the
+// softmax threads and is the A operand of S = Q K^T, so that per KV tile the tensor core reads only
+// K and V from shared memory (an SS MMA would add 32 KB of Q per tile and make the shared-memory
+// pipe the bound).  S is double-buffered: S(it+1) is computed while softmax(it) runs, P(it) (bf16)
+// overwrites the start of each column quarter of S(it) and is the TMEM A operand of O += P V.  The two
+// four softmax warpgroups exchange partial row maxima through shared memory once per KV tile; O is
+// rescaled lazily (only when the running max grew by more than 2^8).
 #pragma once
 #include <cuda.h>
 #include "sm100_ptx.cuh"
@@ -32,6 +32,8 @@
 namespace pf {
 
 struct FwdParams {
+    const __nv_bfloat16* Q;
+    int64_t q_stride_tok, q_stride_head;  // elements
     __nv_bfloat16* O;
     int64_t o_stride_tok, o_stride_head;  // elements
     float* LSE;                           // [Hq, lse_stride], column = packed token row
@@ -44,17 +46,17 @@ struct FwdParams {
 
 template <int D>
 struct FwdCfg {
-    static constexpr int KS = 2;                       // K/V ring depth
+    static constexpr int KS = 3;                       // K/V ring depth
     static constexpr int TILE = 128 * D * 2;           // bytes of one 128 x D bf16 tile
     static constexpr int SUB = 128 * 64 * 2;           // one 128 x 64 swizzle-128B sub-tile
     static constexpr int NSUB = D / 64;
-    static constexpr int OFF_Q = 0;                    // 2 tiles
-    static constexpr int OFF_K = 2 * TILE;             // KS tiles
-    static constexpr int OFF_V = OFF_K + KS * TILE;    // KS tiles
-    static constexpr int OFF_BAR = OFF_V + KS * TILE;
+    static constexpr int OFF_K = 0;                    // KS tiles
+    static constexpr int OFF_V = KS * TILE;            // KS tiles
+    static constexpr int OFF_BAR = 2 * KS * TILE;
     static constexpr int OFF_X = OFF_BAR + 256;        // row-max / row-sum exchange between column halves
-    static constexpr int SMEM = OFF_X + 2 * 2 * 2 * 128 * 4;
+    static constexpr int SMEM = OFF_X + 2 * 4 * 128 * 4;
     static constexpr int THREADS = 576;
+    static constexpr uint32_t T_O = 256, T_Q = 256 + D;  // TMEM columns of O and Q (S[b] at 128 b)
 };
 
 // 2^x for a pair of x <= ~8 on the FMA / ALU pipes (packed f32x2 math): round-to-nearest split
@@ -75,62 +77,59 @@ __device__ __forceinline__ float2 exp2_poly2(float2 x) {
                        __int_as_float(__float_as_int(r.y) + (__float_as_int(t.y) << 23)));
 }
 
+
 template <int D>
 __global__ void __launch_bounds__(576, 1)
-attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK1,
-                const __grid_constant__ CUtensorMap tmV1, const __grid_constant__ CUtensorMap tmK2,
-                const __grid_constant__ CUtensorMap tmV2, const __grid_constant__ FwdParams p) {
+attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant__ CUtensorMap tmV1,
+                const __grid_constant__ CUtensorMap tmK2, const __grid_constant__ CUtensorMap tmV2,
+                const __grid_constant__ FwdParams p) {
     using C = FwdCfg<D>;
     extern __shared__ __align__(1024) uint8_t smem[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::OFF_BAR);
-    uint64_t* bar_Q = bars;                 // [2]
-    uint64_t* bar_Kf = bars + 2;            // [KS]
+    uint64_t* bar_Q = bars;                 // Q written to TMEM by the softmax threads
+    uint64_t* bar_Kf = bars + 1;            // [KS]
     uint64_t* bar_Ke = bars + 4;
-    uint64_t* bar_Vf = bars + 6;
-    uint64_t* bar_Ve = bars + 8;
-    uint64_t* bar_S = bars + 10;            // [2] S_s ready (MMA -> softmax)
-    uint64_t* bar_P = bars + 12;            // [2 slots][2 halves] P_s half ready (softmax -> MMA)
-    uint64_t* bar_done = bars + 16;         // all MMAs complete
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 17);
+    uint64_t* bar_Vf = bars + 7;
+    uint64_t* bar_Ve = bars + 10;
+    uint64_t* bar_S = bars + 13;            // [2] S[b] ready (MMA -> softmax)
+    uint64_t* bar_P = bars + 15;            // [2 buffers][2 halves] P half ready (softmax -> MMA)
+    uint64_t* bar_PV = bars + 19;           // P.V of an iteration complete (needed before O is rescaled)
+    uint64_t* bar_done = bars + 20;         // all MMAs complete
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 22);
 
     const int tid = threadIdx.x, warp = tid >> 5;
     if ((smem_u32(smem) & 1023u) != 0) __trap();
 
-    // ---- work decode: sequence, then its items (rb, h') of KV head g with index rb*G + h',
-    // heaviest (largest rb) first; the two slots of a CTA are consecutive items of one sequence
+    // ---- work decode: sequence, then its items (rb, h') of KV head g, heaviest (largest rb) first
     const int g = blockIdx.y;
     int sq = 0, base = 0, nRB = 0;
     for (;; ++sq) {
         nRB = p.seq.ckt[sq + 1] - p.seq.ckt[sq];
-        const int ncta = (nRB * p.G + 1) >> 1;
-        if (int(blockIdx.x) < base + ncta || sq + 1 >= p.seq.n) break;
-        base += ncta;
+        if (int(blockIdx.x) < base + nRB * p.G || sq + 1 >= p.seq.n) break;
+        base += nRB * p.G;
     }
     const int tok0 = p.seq.cu[sq], Ls = p.seq.cu[sq + 1] - tok0;
-    const int nItems = nRB * p.G;
-    const int idx0 = nItems - 1 - 2 * (int(blockIdx.x) - base);
-    const int idx1 = idx0 - 1;                       // < 0: slot 1 idle
-    const int rb0 = idx0 / p.G, h0 = g * p.G + idx0 % p.G;
-    const int rb1 = idx1 >= 0 ? idx1 / p.G : -1, h1 = idx1 >= 0 ? g * p.G + idx1 % p.G : 0;
+    const int idx = nRB * p.G - 1 - (int(blockIdx.x) - base);
+    const int rb = idx / p.G, h = g * p.G + idx % p.G;
     const int nP = (p.Lp + 127) >> 7;
-    const int n_iter0 = nP + rb0 + 1;                // slot 0 is the longer one
-    const int n_iter1 = idx1 >= 0 ? nP + rb1 + 1 : 0;
+    const int n_iter = nP + rb + 1;
 
     if (tid == 0) {
-        mbar_init(&bar_Q[0], 1); mbar_init(&bar_Q[1], 1);
+        mbar_init(bar_Q, 512);
         for (int s = 0; s < C::KS; ++s) {
             mbar_init(&bar_Kf[s], 1); mbar_init(&bar_Ke[s], 1);
             mbar_init(&bar_Vf[s], 1); mbar_init(&bar_Ve[s], 1);
         }
         mbar_init(&bar_S[0], 1); mbar_init(&bar_S[1], 1);
-        for (int i = 0; i < 4; ++i) mbar_init(&bar_P[i], 128);
+        for (int i = 0; i < 4; ++i) mbar_init(&bar_P[i], 256);
+        mbar_init(bar_PV, 1);
         mbar_init(bar_done, 1);
         fence_mbar_init();
     }
     if (warp == 16) {
         tmem_alloc(tmem_slot, 512);
         if (elect_one()) {
-            tma_prefetch_desc(&tmQ); tma_prefetch_desc(&tmK1); tma_prefetch_desc(&tmV1);
+            tma_prefetch_desc(&tmK1); tma_prefetch_desc(&tmV1);
             tma_prefetch_desc(&tmK2); tma_prefetch_desc(&tmV2);
         }
     }
@@ -142,16 +141,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     if (warp == 16) {
         // =============================== TMA producer ===============================
         if (elect_one()) {
-            mbar_arrive_expect_tx(&bar_Q[0], C::TILE);
-            for (int k = 0; k < C::NSUB; ++k)
-                tma_load_3d(smem + C::OFF_Q + k * C::SUB, &tmQ, &bar_Q[0], 64 * k, h0, tok0 + rb0 * 128);
-            if (idx1 >= 0) {
-                mbar_arrive_expect_tx(&bar_Q[1], C::TILE);
-                for (int k = 0; k < C::NSUB; ++k)
-                    tma_load_3d(smem + C::OFF_Q + C::TILE + k * C::SUB, &tmQ, &bar_Q[1], 64 * k, h1,
-                                tok0 + rb1 * 128);
-            }
-            for (int it = 0; it < n_iter0; ++it) {
+            for (int it = 0; it < n_iter; ++it) {
                 const int st = it % C::KS;
                 const uint32_t ph = (it / C::KS) & 1;
                 const bool pre = it < nP;
@@ -173,209 +163,172 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         if (elect_one()) {
             constexpr uint32_t idesc_qk = make_idesc_bf16(128, 128, false, false);
             constexpr uint32_t idesc_pv = make_idesc_bf16(128, D, false, true);
-            const uint32_t sQ = smem_u32(smem + C::OFF_Q), sK = smem_u32(smem + C::OFF_K),
-                           sV = smem_u32(smem + C::OFF_V);
-            auto issue_S = [&](int s, int st) {  // S_s = Q_s . K^T
-                const uint64_t q = make_smem_desc_sw128(sQ + s * C::TILE, 16, 1024);
+            const uint32_t sK = smem_u32(smem + C::OFF_K), sV = smem_u32(smem + C::OFF_V);
+            auto issue_S = [&](int b, int st) {  // S[b] = Q . K^T   (A = Q from TMEM)
                 const uint64_t k = make_smem_desc_sw128(sK + st * C::TILE, 16, 1024);
 #pragma unroll
-                for (int kk = 0; kk < D / 16; ++kk) {
-                    const uint32_t off = ((kk >> 2) * C::SUB + (kk & 3) * 32) >> 4;
-                    mma_ss(tmem + s * 128, q + off, k + off, idesc_qk, kk > 0);
-                }
+                for (int kk = 0; kk < D / 16; ++kk)
+                    mma_ts(tmem + b * 128, tmem + C::T_Q + kk * 8,
+                           k + (((kk >> 2) * C::SUB + (kk & 3) * 32) >> 4), idesc_qk, kk > 0);
             };
-            auto issue_PV = [&](int s, int st, int half, bool acc) {  // O_s += P_s[:, half] . V[half]
+            auto issue_PV = [&](int b, int st, int half, bool acc) {  // O += P[b][:, half] . V[half]
                 const uint64_t v = make_smem_desc_sw128(sV + st * C::TILE, C::SUB, 1024);
 #pragma unroll
                 for (int kk = half * 4; kk < half * 4 + 4; ++kk)
-                    mma_ts(tmem + 256 + s * D, tmem + s * 128 + half * 64 + (kk & 3) * 8, v + ((kk * 2048) >> 4), idesc_pv,
-                           (acc || kk > 0) ? 1u : 0u);
+                    mma_ts(tmem + C::T_O, tmem + b * 128 + (kk >> 1) * 32 + (kk & 1) * 8,
+                           v + ((kk * 2048) >> 4), idesc_pv, (acc || kk > 0) ? 1u : 0u);
             };
-            mbar_wait(&bar_Q[0], 0);
+            mbar_wait(bar_Q, 0);
             mbar_wait(&bar_Kf[0], 0);
             tc_fence_after();
             issue_S(0, 0);
             mma_commit(&bar_S[0]);
-            if (n_iter1 > 0) {
-                mbar_wait(&bar_Q[1], 0);
-                tc_fence_after();
-                issue_S(1, 0);
-                mma_commit(&bar_S[1]);
-            }
             mma_commit(&bar_Ke[0]);
-            for (int it = 0; it < n_iter0; ++it) {
-                const int st = it % C::KS;
-                const uint32_t ph = (it / C::KS) & 1;
-                const bool next = it + 1 < n_iter0;
-                const int st1 = (it + 1) % C::KS;
-                const uint32_t ph1 = ((it + 1) / C::KS) & 1;
-                mbar_wait(&bar_Vf[st], ph);
-                mbar_wait(&bar_P[0], it & 1);
-                tc_fence_after();
-                issue_PV(0, st, 0, it > 0);
-                mbar_wait(&bar_P[1], it & 1);
-                tc_fence_after();
-                issue_PV(0, st, 1, true);
-                if (next) {
-                    mbar_wait(&bar_Kf[st1], ph1);
+            for (int it = 0; it < n_iter; ++it) {
+                const int st = it % C::KS, b = it & 1;
+                if (it + 1 < n_iter) {   // S(it+1) runs on the tensor pipe while softmax(it) works
+                    const int st1 = (it + 1) % C::KS;
+                    mbar_wait(&bar_Kf[st1], ((it + 1) / C::KS) & 1);
                     tc_fence_after();
-                    issue_S(0, st1);
-                    mma_commit(&bar_S[0]);
-                }
-                if (it < n_iter1) {
-                    mbar_wait(&bar_P[2], it & 1);
-                    tc_fence_after();
-                    issue_PV(1, st, 0, it > 0);
-                    mbar_wait(&bar_P[3], it & 1);
-                    tc_fence_after();
-                    issue_PV(1, st, 1, true);
-                }
-                mma_commit(&bar_Ve[st]);
-                if (next) {
-                    if (it + 1 < n_iter1) {
-                        issue_S(1, st1);
-                        mma_commit(&bar_S[1]);
-                    }
+                    issue_S(b ^ 1, st1);
+                    mma_commit(&bar_S[b ^ 1]);
                     mma_commit(&bar_Ke[st1]);
                 }
+                mbar_wait(&bar_Vf[st], (it / C::KS) & 1);
+                mbar_wait(&bar_P[2 * b], (it >> 1) & 1);
+                tc_fence_after();
+                issue_PV(b, st, 0, it > 0);
+                mbar_wait(&bar_P[2 * b + 1], (it >> 1) & 1);
+                tc_fence_after();
+                issue_PV(b, st, 1, true);
+                mma_commit(&bar_Ve[st]);
+                mma_commit(bar_PV);
             }
             mma_commit(bar_done);
         }
     } else {
         // =============================== softmax warpgroups ===============================
-        const int s = warp >> 3;                 // slot
-        const int hh = (warp >> 2) & 1;          // key-column half of the S tile
+        const int qd = warp >> 2;                // key-column quarter of the S tile / d quarter of Q and O
         const int r = tid & 127;                 // row in tile == TMEM lane
-        const int n_iter = s == 0 ? n_iter0 : n_iter1;
-        const int rb = s == 0 ? rb0 : rb1;
-        const int h = s == 0 ? h0 : h1;
         const int t = rb * 128 + r;              // query row within its sequence
+        const bool valid = t < Ls;
+        constexpr int DQ = D / 4;                // d elements (O columns) per quarter
         const uint32_t lane_off = uint32_t((warp & 3) * 32) << 16;
-        const uint32_t tS = tmem + s * 128 + hh * 64 + lane_off;       // this half of S; P at its start
-        const uint32_t tO = tmem + 256 + s * D + hh * (D / 2) + lane_off;  // this half of the O columns
-        float* xch = reinterpret_cast<float*>(smem + C::OFF_X) + s * 256;  // [parity][slot][half][128]
+        const uint32_t tO = tmem + C::T_O + qd * DQ + lane_off;          // this quarter of the O columns
+        float* xch = reinterpret_cast<float*>(smem + C::OFF_X);          // [parity][quarter][128]
         const float c = p.scale_log2;
+        // ---- Q row -> TMEM (A operand layout: lane = row, column j = elements 2j, 2j+1)
+        {
+            const uint4* qrow = reinterpret_cast<const uint4*>(
+                p.Q + int64_t(tok0 + t) * p.q_stride_tok + int64_t(h) * p.q_stride_head + qd * DQ);
+            uint32_t qv[DQ / 2];
+#pragma unroll
+            for (int j = 0; j < DQ / 8; ++j) {
+                const uint4 v = valid ? qrow[j] : make_uint4(0u, 0u, 0u, 0u);
+                qv[4 * j] = v.x; qv[4 * j + 1] = v.y; qv[4 * j + 2] = v.z; qv[4 * j + 3] = v.w;
+            }
+            if constexpr (D == 128) tmem_st16(tmem + C::T_Q + qd * 16 + lane_off, qv);
+            else tmem_st8(tmem + C::T_Q + qd * 8 + lane_off, qv);
+            tmem_wait_st();
+            tc_fence_before();
+            mbar_arrive(bar_Q);
+        }
         float m_used = -INFINITY, l = 0.f;
         for (int it = 0; it < n_iter; ++it) {
-            mbar_wait(&bar_S[s], it & 1);
+            const int b = it & 1;
+            const uint32_t tS = tmem + b * 128 + qd * 32 + lane_off;     // this quarter of S[b]; P at its start
+            mbar_wait(&bar_S[b], (it >> 1) & 1);
             tc_fence_after();
-            // visible keys of this tile for this row, relative to this half's first column
-            const int limit = (it < nP ? p.Lp - it * 128 : t - (it - nP) * 128 + 1) - hh * 64;
-            const bool masked = limit < 64;      // ragged prefix tail or causal diagonal
-            // ---- pass 1: row maximum (S is read from TMEM twice to keep the live registers low)
-            float mx0 = -INFINITY, mx1 = -INFINITY;
-            {
-                uint32_t x[2][32];
-                tmem_ld32(tS + 0, x[0]);
-                tmem_ld32(tS + 32, x[1]);
-                tmem_wait_ld();
-                if (masked) {
+            uint32_t x[32];
+            tmem_ld32(tS, x);
+            tmem_wait_ld();
+            // visible keys of this tile for this row, relative to this quarter's first column
+            const int limit = (it < nP ? p.Lp - it * 128 : t - (it - nP) * 128 + 1) - qd * 32;
+            if (limit < 32) {                    // ragged prefix tail or causal diagonal
 #pragma unroll
-                    for (int q = 0; q < 2; ++q)
-#pragma unroll
-                        for (int j = 0; j < 32; ++j)
-                            if (q * 32 + j >= limit) x[q][j] = 0xf149f2cau;  // -1e30: exp2 -> 0, stays finite
-                }
-#pragma unroll
-                for (int q = 0; q < 2; ++q)
-#pragma unroll
-                    for (int j = 0; j < 32; j += 2) {
-                        mx0 = fmaxf(mx0, __uint_as_float(x[q][j]));
-                        mx1 = fmaxf(mx1, __uint_as_float(x[q][j + 1]));
-                    }
+                for (int j = 0; j < 32; ++j)
+                    if (j >= limit) x[j] = 0xf149f2cau;  // -1e30: exp2 -> 0, stays finite
             }
-            float* xm = xch + (it & 1) * 512;
-            const float mine = fmaxf(mx0, mx1);
-            xm[hh * 128 + r] = mine;
-            named_bar_sync(1 + s, 256);          // the two warpgroups of the slot
-            const float m_new = fmaxf(mine, xm[(hh ^ 1) * 128 + r]) * c;
+            float mx0 = -INFINITY, mx1 = -INFINITY;
+#pragma unroll
+            for (int j = 0; j < 32; j += 2) {
+                mx0 = fmaxf(mx0, __uint_as_float(x[j]));
+                mx1 = fmaxf(mx1, __uint_as_float(x[j + 1]));
+            }
+            float* xm = xch + b * 512;
+            float mine = fmaxf(mx0, mx1);
+            xm[qd * 128 + r] = mine;
+            named_bar_sync(1, 512);              // the four softmax warpgroups
+#pragma unroll
+            for (int o = 1; o < 4; ++o) mine = fmaxf(mine, xm[((qd + o) & 3) * 128 + r]);
+            const float m_new = mine * c;
             // lazy rescale: keep a stale max while the new one is within 2^8 of it
             const bool need = (it == 0) || (m_new > m_used + 8.f);
             if (__any_sync(0xffffffffu, need && it > 0)) {
+                mbar_wait(bar_PV, (it - 1) & 1); // P.V(it-1) must have landed in O
+                tc_fence_after();
                 const float alpha = need ? fast_exp2(m_used - m_new) : 1.f;
                 l *= alpha;
+                uint32_t o[DQ];
+                if constexpr (D == 128) tmem_ld32(tO, o); else tmem_ld16(tO, o);
+                tmem_wait_ld();
 #pragma unroll
-                for (int q = 0; q < D / 64; ++q) {
-                    uint32_t o[32];
-                    tmem_ld32(tO + q * 32, o);
-                    tmem_wait_ld();
-#pragma unroll
-                    for (int j = 0; j < 32; ++j) o[j] = __float_as_uint(__uint_as_float(o[j]) * alpha);
-                    tmem_st32(tO + q * 32, o);
-                }
+                for (int j = 0; j < DQ; ++j) o[j] = __float_as_uint(__uint_as_float(o[j]) * alpha);
+                if constexpr (D == 128) tmem_st32(tO, o); else tmem_st16(tO, o);
             }
             if (need) m_used = m_new;
-            // ---- pass 2: P = exp2(c S - m), packed to bf16 over the first 32 columns of this half
-            // of S.  Chunk q (columns [32q, 32q+32)) writes P columns [16q, 16q+16): behind the reads.
+            // ---- P = exp2(c S - m), packed to bf16 over the first 16 columns of this quarter of S
             const float2 c2 = make_float2(c, c), nm2 = make_float2(-m_used, -m_used);
             float2 sum2 = make_float2(0.f, 0.f);
-            uint32_t xb[2][32];                  // chunk 1 is in flight while chunk 0 is exponentiated
-            tmem_ld32(tS, xb[0]);
-            tmem_wait_ld();
+            uint32_t pk[16];
 #pragma unroll
-            for (int q = 0; q < 2; ++q) {
-                uint32_t (&x)[32] = xb[q];
-                if (q == 0) tmem_ld32(tS + 32, xb[1]);
-                if (masked) {
-#pragma unroll
-                    for (int j = 0; j < 32; ++j)
-                        if (q * 32 + j >= limit) x[j] = 0xf149f2cau;
+            for (int j = 0; j < 16; ++j) {
+                const float2 a = __ffma2_rn(make_float2(__uint_as_float(x[2 * j]),
+                                                        __uint_as_float(x[2 * j + 1])), c2, nm2);
+                float2 e;
+                if ((j * PF_FWD_POLY16) % 16 < PF_FWD_POLY16) {   // PF_FWD_POLY16 pairs in 16 on the FMA pipe
+                    e = exp2_poly2(a);
+                } else {
+                    e.x = fast_exp2(a.x);
+                    e.y = fast_exp2(a.y);
                 }
-                uint32_t pk[16];
-#pragma unroll
-                for (int j = 0; j < 16; ++j) {
-                    const float2 a = __ffma2_rn(make_float2(__uint_as_float(x[2 * j]),
-                                                            __uint_as_float(x[2 * j + 1])), c2, nm2);
-                    float2 e;
-                    if ((j * PF_FWD_POLY16) % 16 < PF_FWD_POLY16) {   // PF_FWD_POLY16 pairs in 16 on the FMA pipe
-                        e = exp2_poly2(a);
-                    } else {
-                        e.x = fast_exp2(a.x);
-                        e.y = fast_exp2(a.y);
-                    }
-                    sum2 = __fadd2_rn(sum2, e);
-                    pk[j] = pack_bf16(e.x, e.y);
-                }
-                tmem_wait_ld();
-                tmem_st16(tS + q * 16, pk);
+                sum2 = __fadd2_rn(sum2, e);
+                pk[j] = pack_bf16(e.x, e.y);
             }
+            tmem_st16(tS, pk);
             tmem_wait_st();
             tc_fence_before();
-            mbar_arrive(&bar_P[2 * s + hh]);     // this half (64 keys) of P is ready for the MMA warp
+            mbar_arrive(&bar_P[2 * b + (qd >> 1)]);   // this half (64 keys) of P: two quarters arrive
             l += sum2.x + sum2.y;
         }
-        if (n_iter > 0) {
-            // combine the two halves' row sums, then each half normalises its half of the O columns
-            float* xl = xch + (n_iter & 1) * 512;
-            xl[hh * 128 + r] = l;
-            named_bar_sync(1 + s, 256);
-            l += xl[(hh ^ 1) * 128 + r];
-            mbar_wait(bar_done, 0);
-            tc_fence_after();
-            const float inv = 1.f / l;
-            const bool valid = t < Ls;
-            __nv_bfloat16* orow = p.O + int64_t(tok0 + t) * p.o_stride_tok + int64_t(h) * p.o_stride_head +
-                                  hh * (D / 2);
+        // combine the four quarters' row sums, then each quarter normalises its quarter of the O columns
+        float* xl = xch + (n_iter & 1) * 512;
+        xl[qd * 128 + r] = l;
+        named_bar_sync(1, 512);
 #pragma unroll
-            for (int q = 0; q < D / 64; ++q) {
-                uint32_t o[32];
-                tmem_ld32(tO + q * 32, o);
-                tmem_wait_ld();
-                if (valid) {
+        for (int o = 1; o < 4; ++o) l += xl[((qd + o) & 3) * 128 + r];
+        mbar_wait(bar_done, 0);
+        tc_fence_after();
+        const float inv = 1.f / l;
+        __nv_bfloat16* orow = p.O + int64_t(tok0 + t) * p.o_stride_tok + int64_t(h) * p.o_stride_head + qd * DQ;
+        {
+            uint32_t o[DQ];
+            if constexpr (D == 128) tmem_ld32(tO, o); else tmem_ld16(tO, o);
+            tmem_wait_ld();
+            if (valid) {
 #pragma unroll
-                    for (int j = 0; j < 32; j += 8) {
-                        uint4 v;
-                        v.x = pack_bf16(__uint_as_float(o[j + 0]) * inv, __uint_as_float(o[j + 1]) * inv);
-                        v.y = pack_bf16(__uint_as_float(o[j + 2]) * inv, __uint_as_float(o[j + 3]) * inv);
-                        v.z = pack_bf16(__uint_as_float(o[j + 4]) * inv, __uint_as_float(o[j + 5]) * inv);
-                        v.w = pack_bf16(__uint_as_float(o[j + 6]) * inv, __uint_as_float(o[j + 7]) * inv);
-                        *reinterpret_cast<uint4*>(orow + q * 32 + j) = v;
-                    }
+                for (int j = 0; j < DQ; j += 8) {
+                    uint4 v;
+                    v.x = pack_bf16(__uint_as_float(o[j + 0]) * inv, __uint_as_float(o[j + 1]) * inv);
+                    v.y = pack_bf16(__uint_as_float(o[j + 2]) * inv, __uint_as_float(o[j + 3]) * inv);
+                    v.z = pack_bf16(__uint_as_float(o[j + 4]) * inv, __uint_as_float(o[j + 5]) * inv);
+                    v.w = pack_bf16(__uint_as_float(o[j + 6]) * inv, __uint_as_float(o[j + 7]) * inv);
+                    *reinterpret_cast<uint4*>(orow + j) = v;
                 }
             }
-            if (valid && hh == 0)
-                p.LSE[int64_t(h) * p.lse_stride + tok0 + t] = (m_used + log2f(l)) * 0.6931471805599453f;
         }
+        if (valid && qd == 0)
+            p.LSE[int64_t(h) * p.lse_stride + tok0 + t] = (m_used + log2f(l)) * 0.6931471805599453f;
     }
     tc_fence_before();
     __syncthreads();

@@ -249,9 +249,8 @@ pf_status launch_fwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const
     pf_ctx* ctx = g->ctx;
     const int Hq = g->desc.n_q_heads, Hkv = g->desc.n_kv_heads;
     const int64_t total = cu[n];
-    CUtensorMap mQ, mK1, mV1, mK2, mV2;
+    CUtensorMap mK1, mV1, mK2, mV2;
     pf_status st;
-    if ((st = make_map(ctx, &mQ, "Q", Q, total, Hq, D))) return st;
     if ((st = make_map(ctx, &mK2, "K", K2, total, Hkv, D))) return st;
     if ((st = make_map(ctx, &mV2, "V", V2, total, Hkv, D))) return st;
     if (Lp > 0) {
@@ -262,6 +261,9 @@ pf_status launch_fwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const
         mV1 = mV2;
     }
     pf::FwdParams p;
+    p.Q = static_cast<const __nv_bfloat16*>(Q.ptr);
+    p.q_stride_tok = Q.stride_tok;
+    p.q_stride_head = Q.stride_head;
     p.O = static_cast<__nv_bfloat16*>(O.ptr);
     p.o_stride_tok = O.stride_tok;
     p.o_stride_head = O.stride_head;
@@ -274,13 +276,13 @@ pf_status launch_fwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const
     p.scale_log2 = g->sigma * 1.4426950408889634f;
     p.seq = make_seq_table(n, cu);
     int ctas = 0;
-    for (int i = 0; i < n; ++i) ctas += ((p.seq.ckt[i + 1] - p.seq.ckt[i]) * p.G + 1) / 2;
+    for (int i = 0; i < n; ++i) ctas += (p.seq.ckt[i + 1] - p.seq.ckt[i]) * p.G;
     if (ctas == 0) return PF_OK;
     dim3 grid(ctas, Hkv);
     {
         ProfScope prof(ctx, prof_kind, s);
         pf::attn_fwd_kernel<D><<<grid, pf::FwdCfg<D>::THREADS, pf::FwdCfg<D>::SMEM, s>>>(
-            mQ, mK1, mV1, mK2, mV2, p);
+            mK1, mV1, mK2, mV2, p);
     }
     PF_CUDA(ctx, cudaGetLastError());
     ctx->n_launches += 1;
