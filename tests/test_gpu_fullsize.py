@@ -61,3 +61,53 @@ def test_config_7b_sampled():
     dk_own, dv_own = oref.cols(q1, k1, v1, do1, lse_f, dl_f, np.full(len(pj), kv, np.int32), pj, 0, Lp)
     check("dK1 = own + gK1, sampled keys", g.dK1[pj, kv], dk_own + gk_sum)
     check("dV1 = own + gV1, sampled keys", g.dV1[pj, kv], dv_own + gv_sum)
+
+
+def _phaseB_subset_sampled(shape, subset, kv, pj, sj_of):
+    """Phase A + Phase B of a SUBSET of the config's suffixes in one packed wave (the prefix and the
+    chosen suffixes are drawn exactly as in the full config); every suffix row of KV-head group `kv`
+    and sampled key columns are compared, gK1/gV1 against the sum over the subset."""
+    inp = inputs.make_group(shape, only_suffixes=subset)
+    G, d = shape.G, shape.head_dim
+    ctx = pf.pf_create(0)
+    g = schedule.to_device(inp, suffixes=subset, wave=len(subset))
+    grp = pf.pf_group_begin(ctx, g.desc, g.Lp, g.K1, g.V1, g.gK1, g.gV1, g.workspace)
+    pf.pf_phaseA_fwd(grp, g.Q1, g.O1, g.LSE1)
+    pk = g.packed[0]
+    pf.pf_phaseB_fwd(grp, pk["cu"], pk["Q2"], pk["K2"], pk["V2"], pk["O2"], pk["LSE2"])
+    pf.pf_phaseB_bwd(grp, pk["cu"], pk["Q2"], pk["K2"], pk["V2"], pk["O2"], pk["LSE2"], pk["dO2"],
+                     pk["dQ2"], pk["dK2"], pk["dV2"])
+    pf.pf_group_end(grp)
+    torch.cuda.synchronize()
+    pf.pf_destroy(ctx)
+    heads = list(range(kv * G, (kv + 1) * G))
+    gk_sum = np.zeros((len(pj), d)); gv_sum = np.zeros((len(pj), d))
+    for n, i in enumerate(subset):
+        sj = sj_of(shape.Ls[i])
+        r = oref.sampled_phaseB(inp, i, kv, pj, sj)
+        gk_sum += r["gk"]; gv_sum += r["gv"]
+        check(f"O2[{i}]", g.O2[n][:, heads].permute(1, 0, 2), r["o2"])
+        check(f"LSE2[{i}]", g.LSE2[n][heads], r["lse2"], lse=True)
+        check(f"dQ2[{i}]", g.dQ2[n][:, heads].permute(1, 0, 2), r["dq2"])
+        check(f"dK2[{i}] sampled keys", g.dK2[n][sj, kv], r["dk2"])
+        check(f"dV2[{i}] sampled keys", g.dV2[n][sj, kv], r["dv2"])
+    check("gK1 (subset), sampled keys", g.gK1[pj, kv], gk_sum)
+    check("gV1 (subset), sampled keys", g.gV1[pj, kv], gv_sum)
+
+
+def test_config_ragged_sampled():
+    """BASELINE.json configs[2]: 28q/4kv, prefix 16384, ragged suffix lengths (three of the 16)."""
+    shape = inputs.config_ragged()
+    order = np.argsort(shape.Ls)
+    subset = sorted(int(i) for i in (order[0], order[len(order) // 2], order[-1]))   # shortest, median, longest
+    pj = np.array([0, 127, 128, 8191, 8192, 12345, 16255, 16256, 16383], dtype=np.int64)
+    sj_of = lambda Ls: np.unique(np.array([0, 1, 63, 64, 127, 128, Ls // 2, Ls - 2, Ls - 1], dtype=np.int64))
+    _phaseB_subset_sampled(shape, subset, kv=2, pj=pj, sj_of=sj_of)
+
+
+def test_config_32k_sampled():
+    """BASELINE.json configs[4]: 40q/8kv (GQA 5:1), prefix 32768, one of the 8 suffixes of 2048."""
+    shape = inputs.config_32k()
+    pj = np.array([0, 128, 16383, 16384, 32639, 32640, 32767], dtype=np.int64)
+    sj_of = lambda Ls: np.array([0, 127, 128, 1024, Ls - 1], dtype=np.int64)
+    _phaseB_subset_sampled(shape, [3], kv=5, pj=pj, sj_of=sj_of)
