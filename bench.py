@@ -249,6 +249,7 @@ def main() -> None:
     ap.add_argument("--no-wave1", action="store_true", help="skip the extra wave = 1 measurement")
     ap.add_argument("--no-offload", action="store_true", help="skip the memory-lifecycle / offload measurement")
     ap.add_argument("--offload-wave", type=int, default=1, help="suffixes per wave in the lifecycle measurement")
+    ap.add_argument("--layers", type=int, default=4, help="attention layers in the multi-layer offload pipeline (0 = skip)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -406,6 +407,23 @@ def main() -> None:
                       note="one attention layer; tensors allocated and freed as a trainer would "
                            "(suffix-wave tensors live only during their wave); peaks are "
                            "torch.cuda.max_memory_allocated")
+        if args.layers > 0:
+            # L layers (independent seeded groups of the same shape), offload pipeline with
+            # one-layer-ahead prefetch before Phase C
+            layers = [inp] + [inputs.make_group(pfd.rank_shape(shape, 1000 + l)) for l in range(1, args.layers)]
+            ml = {}
+            for mode in (False, True):
+                schedule.run_multilayer_step(ctx, layers, dev, wave=args.offload_wave, offload=mode, pinned=pinned)
+                r = schedule.run_multilayer_step(ctx, layers, dev, wave=args.offload_wave, offload=mode, pinned=pinned)
+                r.pop("outputs")
+                ml["offload" if mode else "resident"] = r
+                torch.cuda.empty_cache()
+            memory["multilayer"] = dict(
+                layers=args.layers, resident=ml["resident"], offload=ml["offload"],
+                phaseB_peak_reduction_pct=100.0 * (1 - ml["offload"]["peak_phaseB_bytes"] / ml["resident"]["peak_phaseB_bytes"]),
+                exposed_prefetch_ms=ml["offload"]["exposed_prefetch_ms"])
+            del layers
+        pinned.clear()
         g = schedule.to_device(inp, dev, wave=wave)
 
     # ---- end to end: pinned host inputs -> device, step, results -> pinned host, every step ----

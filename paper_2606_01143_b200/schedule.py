@@ -258,3 +258,138 @@ def run_lifecycle_step(ctx, inp, device="cuda", wave: int = 1, offload: bool = T
         outs.update(dQ1=dQ1, dK1=dK1, dV1=dV1)
     return dict(ms=t0.elapsed_time(t1), peak_step_bytes=max(peak_a, torch.cuda.max_memory_allocated(dev)),
                 peak_phaseB_bytes=peak_b, resident_at_phaseB_start_bytes=base, outputs=outs)
+
+
+# --------------------------------------------------------------------------------------------------
+# Multi-layer lifecycle: L attention layers, each with
+# its own training-time KV cache.  Phase A runs layer by layer and every layer's dormant set
+# {Q1, O1, LSE1} leaves for the pinned host pool on the side stream as soon as it is produced;
+# Phase B runs all waves on all layers with only the hot sets {K1, V1, gK1, gV1} resident; Phase C
+# runs in reverse layer order with the dormant set of layer l-1 prefetched while layer l computes
+# (if a prefetch has not been issued or has not landed, Phase C simply waits for it: demand load).
+# --------------------------------------------------------------------------------------------------
+def run_multilayer_step(ctx, layers, device="cuda", wave: int = 1, offload: bool = True,
+                        pinned: Optional[dict] = None, keep_outputs: bool = False) -> dict:
+    """`layers`: list of inputs.GroupInputs with identical shapes (one per attention layer)."""
+    s = layers[0].shape
+    dev = torch.device(device)
+    Hq, Hkv, d, Lp, L = s.n_q_heads, s.n_kv_heads, s.head_dim, s.Lp, len(layers)
+    bf, f32 = torch.bfloat16, torch.float32
+    main = torch.cuda.current_stream(dev)
+    pinned = pinned if pinned is not None else {}
+    side = pinned.setdefault("side_stream", torch.cuda.Stream(dev))
+    e = lambda n, H, dt=bf: torch.empty((n, H, d), dtype=dt, device=dev)
+    waves = _waves(s.N, wave)
+    max_tok = max((sum(s.Ls[k] for k in w) for w in waves), default=0)
+    desc = pf.make_desc(Hq, Hkv, d)
+
+    def pin(l, name, like):
+        key = (l, name)
+        if key not in pinned:
+            pinned[key] = torch.empty(like.shape, dtype=like.dtype, pin_memory=True)
+        return pinned[key]
+
+    torch.cuda.synchronize(dev)
+    torch.cuda.reset_peak_memory_stats(dev)
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record(main)
+    ws = torch.empty(pf.pf_workspace_bytes(desc, Lp, max_tok), dtype=torch.uint8, device=dev)
+    hot, dorm, grp, outs = [], [], [], [dict() for _ in range(L)]
+    exposed = []                                    # (event before wait, event after wait) per layer
+    try:
+        # ---- Phase A, layer by layer; dormant sets stream out behind it
+        for l, inp in enumerate(layers):
+            Q1, K1, V1 = inp.Q1.to(dev), inp.K1.to(dev), inp.V1.to(dev)
+            O1 = e(Lp, Hq); LSE1 = torch.empty((Hq, Lp), dtype=f32, device=dev)
+            gK1, gV1 = e(Lp, Hkv, f32), e(Lp, Hkv, f32)
+            g = pf.pf_group_begin(ctx, desc, Lp, K1, V1, gK1, gV1, ws, main)
+            grp.append(g)
+            pf.pf_phaseA_fwd(g, Q1, O1, LSE1, main)
+            hot.append(dict(K1=K1, V1=V1, gK1=gK1, gV1=gV1))
+            dset = dict(Q1=Q1, O1=O1, LSE1=LSE1)
+            if keep_outputs:
+                outs[l]["O1"], outs[l]["LSE1"] = O1.clone(), LSE1.clone()
+            if offload:
+                ev = torch.cuda.Event(); ev.record(main)
+                side.wait_event(ev)
+                for name, t in dset.items():
+                    pf.pf_offload(ctx, t, pin(l, name, t), side)
+                dset = dict(shapes={k: (t.shape, t.dtype) for k, t in dset.items()},
+                            done=torch.cuda.Event())
+                dset["done"].record(side)
+                dset["keep"] = (Q1, O1, LSE1)       # freed once the copy has left (below)
+            dorm.append(dset)
+            del Q1, O1, LSE1
+        if offload:
+            side.synchronize()                      # all dormant sets are on the host: free them
+            for dset in dorm:
+                dset.pop("keep")
+        peak_a = torch.cuda.max_memory_allocated(dev)
+        torch.cuda.reset_peak_memory_stats(dev)
+        base = torch.cuda.memory_allocated(dev)
+        # ---- Phase B: every wave on every layer (a wave's tensors live only during the wave)
+        for w in waves:
+            cu = [0]
+            for k in w:
+                cu.append(cu[-1] + s.Ls[k])
+            tot = cu[-1]
+            for l, inp in enumerate(layers):
+                cat = lambda src: torch.cat([src[k] for k in w], 0).contiguous().to(dev)
+                Q2, K2, V2, dO2 = cat(inp.Q2), cat(inp.K2), cat(inp.V2), cat(inp.dO2)
+                O2, dQ2, dK2, dV2 = e(tot, Hq), e(tot, Hq), e(tot, Hkv), e(tot, Hkv)
+                LSE2 = torch.empty((Hq, tot), dtype=f32, device=dev)
+                pf.pf_phaseB_fwd(grp[l], cu, Q2, K2, V2, O2, LSE2, main)
+                pf.pf_phaseB_bwd(grp[l], cu, Q2, K2, V2, O2, LSE2, dO2, dQ2, dK2, dV2, main)
+                if keep_outputs:
+                    for j, k in enumerate(w):
+                        sl = slice(cu[j], cu[j + 1])
+                        outs[l][f"O2[{k}]"], outs[l][f"LSE2[{k}]"] = O2[sl].clone(), LSE2[:, sl].clone()
+                        outs[l][f"dQ2[{k}]"], outs[l][f"dK2[{k}]"], outs[l][f"dV2[{k}]"] = (
+                            dQ2[sl].clone(), dK2[sl].clone(), dV2[sl].clone())
+                del Q2, K2, V2, dO2, O2, dQ2, dK2, dV2, LSE2
+        peak_b = torch.cuda.max_memory_allocated(dev)
+
+        # ---- Phase C in reverse layer order, prefetching one layer ahead
+        def prefetch(l):
+            dset = dorm[l]
+            ev = torch.cuda.Event(); ev.record(main)   # fresh buffers may reuse blocks main still reads
+            bufs = {k: torch.empty(sh, dtype=dt, device=dev) for k, (sh, dt) in dset["shapes"].items()}
+            side.wait_event(ev)
+            for name, t in bufs.items():
+                pf.pf_prefetch(ctx, pinned[(l, name)], t, side)
+            dset["bufs"], dset["landed"] = bufs, torch.cuda.Event()
+            dset["landed"].record(side)
+
+        if offload:
+            prefetch(L - 1)
+        for l in range(L - 1, -1, -1):
+            if offload:
+                if "bufs" not in dorm[l]:
+                    prefetch(l)                       # demand load: nobody prefetched this layer
+                b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                b0.record(main)
+                main.wait_event(dorm[l]["landed"])
+                b1.record(main)
+                exposed.append((b0, b1))
+                if l > 0:
+                    prefetch(l - 1)                   # overlaps Phase C of layer l
+                Q1, O1, LSE1 = (dorm[l]["bufs"][k] for k in ("Q1", "O1", "LSE1"))
+            else:
+                Q1, O1, LSE1 = (dorm[l][k] for k in ("Q1", "O1", "LSE1"))
+            dO1 = layers[l].dO1.to(dev)
+            dQ1, dK1, dV1 = e(Lp, Hq), e(Lp, Hkv), e(Lp, Hkv)
+            pf.pf_phaseC_bwd(grp[l], Q1, O1, LSE1, dO1, dQ1, dK1, dV1, main)
+            if keep_outputs:
+                outs[l].update(dQ1=dQ1, dK1=dK1, dV1=dV1)
+            dorm[l] = None
+            hot[l] = None
+            del Q1, O1, LSE1, dO1, dQ1, dK1, dV1
+    finally:
+        for g in grp:
+            pf.pf_group_end(g)
+    t1.record(main)
+    torch.cuda.synchronize(dev)
+    return dict(ms=t0.elapsed_time(t1), layers=L,
+                peak_step_bytes=max(peak_a, peak_b, torch.cuda.max_memory_allocated(dev)),
+                peak_phaseB_bytes=peak_b, resident_at_phaseB_start_bytes=base,
+                exposed_prefetch_ms=sum(a.elapsed_time(b) for a, b in exposed), outputs=outs)

@@ -264,3 +264,24 @@ def test_memory_lifecycle_offload(ctx, offload):
         base = schedule.run_lifecycle_step(ctx, inp, wave=2, offload=False)
         assert r["resident_at_phaseB_start_bytes"] < base["resident_at_phaseB_start_bytes"]
         assert r["peak_phaseB_bytes"] < base["peak_phaseB_bytes"]
+
+
+@pytest.mark.parametrize("offload", [False, True])
+def test_multilayer_offload_pipeline(ctx, offload):
+    """L layers of caches, dormant sets offloaded as produced, Phase C in reverse
+    layer order with one-layer-ahead prefetch.  Every layer must still match its oracle."""
+    shapes = [inputs.small_case(4, 2, 128, 300, [130, 64, 70], seed=50 + l, dist="unit") for l in range(3)]
+    layers = [inputs.make_group(s) for s in shapes]
+    r = schedule.run_multilayer_step(ctx, layers, wave=2, offload=offload, keep_outputs=True)
+    for l, inp in enumerate(layers):
+        ref = oracle.group_reference(inp)
+        o = r["outputs"][l]
+        check(f"L{l} O1", o["O1"], ref.O1); check(f"L{l} LSE1", o["LSE1"], ref.LSE1, lse=True)
+        for i in range(shapes[l].N):
+            check(f"L{l} O2[{i}]", o[f"O2[{i}]"], ref.O2[i])
+            check(f"L{l} dQ2[{i}]", o[f"dQ2[{i}]"], ref.dQ2[i])
+            check(f"L{l} dK2[{i}]", o[f"dK2[{i}]"], ref.dK2[i]); check(f"L{l} dV2[{i}]", o[f"dV2[{i}]"], ref.dV2[i])
+        check(f"L{l} dQ1", o["dQ1"], ref.dQ1); check(f"L{l} dK1", o["dK1"], ref.dK1); check(f"L{l} dV1", o["dV1"], ref.dV1)
+    if offload:
+        base = schedule.run_multilayer_step(ctx, layers, wave=2, offload=False)
+        assert r["peak_phaseB_bytes"] < base["peak_phaseB_bytes"]
