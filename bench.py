@@ -422,6 +422,11 @@ def main() -> None:
                 layers=args.layers, resident=ml["resident"], offload=ml["offload"],
                 phaseB_peak_reduction_pct=100.0 * (1 - ml["offload"]["peak_phaseB_bytes"] / ml["resident"]["peak_phaseB_bytes"]),
                 exposed_prefetch_ms=ml["offload"]["exposed_prefetch_ms"])
+            r = schedule.run_multilayer_step(ctx, layers, dev, wave=args.offload_wave, offload=True, pinned=pinned,
+                                             early_prefetch=True)
+            memory["multilayer"]["early_prefetch"] = dict(
+                phaseB_peak_reduction_pct=100.0 * (1 - r["peak_phaseB_bytes"] / ml["resident"]["peak_phaseB_bytes"]),
+                exposed_prefetch_ms=r["exposed_prefetch_ms"], ms=r["ms"])
             del layers
         pinned.clear()
         g = schedule.to_device(inp, dev, wave=wave)

@@ -94,6 +94,38 @@ dq_finish_kernel(const float* __restrict__ acc, __nv_bfloat16* __restrict__ dst,
     }
 }
 
+// Two fp32 accumulators [L, H, D] contiguous (dK and dV) -> two bf16 strided outputs in one launch:
+// blockIdx.y selects the pair; dst = bf16_rne(src)
+template <int D>
+__global__ void __launch_bounds__(256)
+acc2_to_bf16_kernel(const float* __restrict__ src0, __nv_bfloat16* __restrict__ dst0, int64_t st0,
+                    int64_t sh0, const float* __restrict__ src1, __nv_bfloat16* __restrict__ dst1,
+                    int64_t st1, int64_t sh1, int64_t L, int H) {
+    constexpr int TPR = D / 8;
+    const bool second = blockIdx.y != 0;
+    const float* src = second ? src1 : src0;
+    __nv_bfloat16* dst = second ? dst1 : dst0;
+    const int64_t d_st = second ? st1 : st0, d_sh = second ? sh1 : sh0;
+    const int64_t gid = int64_t(blockIdx.x) * 256 + threadIdx.x;
+    const int64_t row = gid / TPR;  // t * H + h
+    const int c = int(gid % TPR);
+    if (row >= L * H) return;
+    const int64_t t = row / H;
+    const int h = int(row % H);
+    const float4 a = *reinterpret_cast<const float4*>(src + row * D + c * 8);
+    const float4 b = *reinterpret_cast<const float4*>(src + row * D + c * 8 + 4);
+    __nv_bfloat162 p0 = __floats2bfloat162_rn(a.x, a.y);
+    __nv_bfloat162 p1 = __floats2bfloat162_rn(a.z, a.w);
+    __nv_bfloat162 p2 = __floats2bfloat162_rn(b.x, b.y);
+    __nv_bfloat162 p3 = __floats2bfloat162_rn(b.z, b.w);
+    uint4 v;
+    v.x = *reinterpret_cast<uint32_t*>(&p0);
+    v.y = *reinterpret_cast<uint32_t*>(&p1);
+    v.z = *reinterpret_cast<uint32_t*>(&p2);
+    v.w = *reinterpret_cast<uint32_t*>(&p3);
+    *reinterpret_cast<uint4*>(dst + t * d_st + int64_t(h) * d_sh + c * 8) = v;
+}
+
 // src fp32 [L, H, D] contiguous -> dst bf16 [L, H, D] strided, dst = bf16_rne(src * scale)
 template <int D>
 __global__ void __launch_bounds__(256)

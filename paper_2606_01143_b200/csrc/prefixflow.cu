@@ -387,14 +387,16 @@ pf_status launch_bwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const
     return PF_OK;
 }
 
+// dK, dV fp32 accumulators -> bf16 outputs, one launch for the pair
 template <int D>
-pf_status launch_convert_kv(pf_group* g, const float* acc, const pf_tensor& dst, int64_t L,
-                            cudaStream_t s) {
+pf_status launch_convert_kv2(pf_group* g, const float* accK, const pf_tensor& dK, const float* accV,
+                             const pf_tensor& dV, int64_t L, cudaStream_t s) {
     const int Hkv = g->desc.n_kv_heads;
     const int64_t threads = L * Hkv * (D / 8);
     if (threads == 0) return PF_OK;
-    pf::acc_to_bf16_kernel<D><<<unsigned((threads + 255) / 256), 256, 0, s>>>(
-        acc, static_cast<__nv_bfloat16*>(dst.ptr), dst.stride_tok, dst.stride_head, L, Hkv, 1.0f);
+    pf::acc2_to_bf16_kernel<D><<<dim3(unsigned((threads + 255) / 256), 2), 256, 0, s>>>(
+        accK, static_cast<__nv_bfloat16*>(dK.ptr), dK.stride_tok, dK.stride_head, accV,
+        static_cast<__nv_bfloat16*>(dV.ptr), dV.stride_tok, dV.stride_head, L, Hkv);
     PF_CUDA(g->ctx, cudaGetLastError());
     g->ctx->n_launches += 1;
     return PF_OK;
@@ -702,13 +704,11 @@ pf_status pf_phaseB_bwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens
         if (d == 64) {
             st = launch_bwd<64>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, dout,
                                 grp->gK1, grp->gV1, ak, av, dq, n, cu, 2, s);
-            if (!st) st = launch_convert_kv<64>(grp, ak, tok_offset(dK2, t0), tot, s);
-            if (!st) st = launch_convert_kv<64>(grp, av, tok_offset(dV2, t0), tot, s);
+            if (!st) st = launch_convert_kv2<64>(grp, ak, tok_offset(dK2, t0), av, tok_offset(dV2, t0), tot, s);
         } else {
             st = launch_bwd<128>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, dout,
                                  grp->gK1, grp->gV1, ak, av, dq, n, cu, 2, s);
-            if (!st) st = launch_convert_kv<128>(grp, ak, tok_offset(dK2, t0), tot, s);
-            if (!st) st = launch_convert_kv<128>(grp, av, tok_offset(dV2, t0), tot, s);
+            if (!st) st = launch_convert_kv2<128>(grp, ak, tok_offset(dK2, t0), av, tok_offset(dV2, t0), tot, s);
         }
         if (st) return st;
     }
@@ -748,13 +748,11 @@ pf_status pf_phaseC_bwd(pf_group* grp, pf_tensor Q1, pf_tensor O1, const float* 
         if (d == 64) {
             st = launch_bwd<64>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, dO1, nullptr,
                                 nullptr, ak, av, dQ1, 1, cu, 3, s);
-            if (!st) st = launch_convert_kv<64>(grp, ak, dK1, Lp, s);
-            if (!st) st = launch_convert_kv<64>(grp, av, dV1, Lp, s);
+            if (!st) st = launch_convert_kv2<64>(grp, ak, dK1, av, dV1, Lp, s);
         } else {
             st = launch_bwd<128>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, dO1, nullptr,
                                  nullptr, ak, av, dQ1, 1, cu, 3, s);
-            if (!st) st = launch_convert_kv<128>(grp, ak, dK1, Lp, s);
-            if (!st) st = launch_convert_kv<128>(grp, av, dV1, Lp, s);
+            if (!st) st = launch_convert_kv2<128>(grp, ak, dK1, av, dV1, Lp, s);
         }
         if (st) return st;
     }

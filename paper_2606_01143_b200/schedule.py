@@ -269,8 +269,11 @@ def run_lifecycle_step(ctx, inp, device="cuda", wave: int = 1, offload: bool = T
 # (if a prefetch has not been issued or has not landed, Phase C simply waits for it: demand load).
 # --------------------------------------------------------------------------------------------------
 def run_multilayer_step(ctx, layers, device="cuda", wave: int = 1, offload: bool = True,
-                        pinned: Optional[dict] = None, keep_outputs: bool = False) -> dict:
-    """`layers`: list of inputs.GroupInputs with identical shapes (one per attention layer)."""
+                        pinned: Optional[dict] = None, keep_outputs: bool = False,
+                        early_prefetch: bool = False) -> dict:
+    """`layers`: list of inputs.GroupInputs with identical shapes (one per attention layer).
+    `early_prefetch` issues the first Phase-C prefetch behind the last Phase-B wave: no exposed wait,
+    but its buffers count in the Phase-B peak."""
     s = layers[0].shape
     dev = torch.device(device)
     Hq, Hkv, d, Lp, L = s.n_q_heads, s.n_kv_heads, s.head_dim, s.Lp, len(layers)
@@ -327,8 +330,20 @@ def run_multilayer_step(ctx, layers, device="cuda", wave: int = 1, offload: bool
         peak_a = torch.cuda.max_memory_allocated(dev)
         torch.cuda.reset_peak_memory_stats(dev)
         base = torch.cuda.memory_allocated(dev)
+        def prefetch(l):
+            dset = dorm[l]
+            ev = torch.cuda.Event(); ev.record(main)   # fresh buffers may reuse blocks main still reads
+            bufs = {k: torch.empty(sh, dtype=dt, device=dev) for k, (sh, dt) in dset["shapes"].items()}
+            side.wait_event(ev)
+            for name, t in bufs.items():
+                pf.pf_prefetch(ctx, pinned[(l, name)], t, side)
+            dset["bufs"], dset["landed"] = bufs, torch.cuda.Event()
+            dset["landed"].record(side)
+
         # ---- Phase B: every wave on every layer (a wave's tensors live only during the wave)
-        for w in waves:
+        for wi, w in enumerate(waves):
+            if offload and early_prefetch and wi == len(waves) - 1:
+                prefetch(L - 1)                       # hidden behind the last wave (costs its buffers in the Phase-B peak)
             cu = [0]
             for k in w:
                 cu.append(cu[-1] + s.Ls[k])
@@ -350,17 +365,7 @@ def run_multilayer_step(ctx, layers, device="cuda", wave: int = 1, offload: bool
         peak_b = torch.cuda.max_memory_allocated(dev)
 
         # ---- Phase C in reverse layer order, prefetching one layer ahead
-        def prefetch(l):
-            dset = dorm[l]
-            ev = torch.cuda.Event(); ev.record(main)   # fresh buffers may reuse blocks main still reads
-            bufs = {k: torch.empty(sh, dtype=dt, device=dev) for k, (sh, dt) in dset["shapes"].items()}
-            side.wait_event(ev)
-            for name, t in bufs.items():
-                pf.pf_prefetch(ctx, pinned[(l, name)], t, side)
-            dset["bufs"], dset["landed"] = bufs, torch.cuda.Event()
-            dset["landed"].record(side)
-
-        if offload:
+        if offload and "bufs" not in dorm[L - 1]:
             prefetch(L - 1)
         for l in range(L - 1, -1, -1):
             if offload:
