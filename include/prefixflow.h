@@ -76,7 +76,10 @@ const char* pf_last_error(const pf_ctx* ctx);
  *                      All pairs in one CTA = that key tile's gK1/gV1 rows are added by one CTA
  *                      (no contention); 1 = maximal parallelism, most reduce-add traffic.
  *   "bwd_heads_per_item" : the same for the tiles of a suffix's own (causal) keys: query heads of
- *                      the KV head per CTA (0 = heuristic). */
+ *                      the KV head per CTA (0 = heuristic).
+ *   "zero_accumulators"  : 1 (default) = pf_group_begin zeroes gK1/gV1; 0 = it leaves them as they
+ *                      are (segment-by-segment training, where they already hold the contributions
+ *                      of later segments). */
 pf_status pf_set_option(pf_ctx* ctx, const char* name, int64_t value);
 
 /*   "profile"        : 1 = bracket every attention kernel launch (not the elementwise helpers)
@@ -103,7 +106,8 @@ size_t pf_workspace_bytes(const pf_desc* desc, int64_t Lp, int64_t max_Ls);
  * asynchronously on `stream`).  gK1.ptr and gV1.ptr may both be NULL: then
  * Phase B is not allowed and Phase C runs without injection (the N-times replay baseline).
  * `workspace` must be 256-byte aligned device memory of >= pf_workspace_bytes(desc, Lp, max_Ls)
- * for every later call of this group; it may be shared by groups that never overlap in time. */
+ * for every later call of this group (each call checks the capacity it needs: Phase C Lp rows, a
+ * Phase-B wave or a segment its own rows -> PF_WORKSPACE); it may be shared by groups that never overlap in time. */
 pf_status pf_group_begin(pf_ctx* ctx, const pf_desc* desc, int64_t Lp, pf_tensor K1, pf_tensor V1,
                          pf_tensor gK1, pf_tensor gV1, void* workspace, size_t workspace_bytes,
                          void* stream, pf_group** out);
@@ -135,6 +139,24 @@ pf_status pf_phaseB_bwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens
  * and rounded once.  Side effect: on return gK1/gV1 hold that fp32 sum. */
 pf_status pf_phaseC_bwd(pf_group* grp, pf_tensor Q1, pf_tensor O1, const float* LSE1,
                         pf_tensor dO1, pf_tensor dQ1, pf_tensor dK1, pf_tensor dV1, void* stream);
+
+/* Segment-by-segment training of ONE long sequence ("a long single sequence can train
+ * segment by segment, accumulating gK/gV into earlier segments as Proposition 3.1 prescribes").
+ * Segment k is the "suffix" of a group whose prefix [0, Lp) is the concatenation of segments < k:
+ * K1/V1 = their keys/values (borrowed in place), gK1/gV1 = rows [0, Lp) of a sequence-wide fp32
+ * accumulator [L, Hkv, d] (open the group with option "zero_accumulators" = 0).
+ *   pf_group_mark_cached : declares K1/V1 valid without running Phase A (they were produced when the
+ *                          earlier segments ran), so that pf_phaseB_fwd may be called for the segment.
+ *   pf_segment_bwd       : backward of the segment.  dQ [Ls,Hq,d] bf16; gK1/gV1 += the gradients that
+ *                          reach the earlier segments' keys (exactly pf_phaseB_bwd); the segment's own
+ *                          key rows accumulate into accK/accV (fp32, contiguous [Ls,Hkv,d]: the
+ *                          accumulator rows of THIS segment, which hold the contributions of the later
+ *                          segments on entry) and dK, dV = bf16(accK), bf16(accV) on exit -- one rounding.
+ * Run the segments in order for the forward and in reverse order for the backward. */
+pf_status pf_group_mark_cached(pf_group* grp);
+pf_status pf_segment_bwd(pf_group* grp, int64_t Ls, pf_tensor Q, pf_tensor K, pf_tensor V, pf_tensor O,
+                         const float* LSE, pf_tensor dO, pf_tensor dQ, float* accK, float* accV,
+                         pf_tensor dK, pf_tensor dV, void* stream);
 
 /* Close the group (host-side; frees the handle only; enqueued work keeps running). */
 pf_status pf_group_end(pf_group* grp);

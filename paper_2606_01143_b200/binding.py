@@ -24,7 +24,7 @@ STATUS_NAMES = {0: "PF_OK", 1: "PF_INVALID_ARG", 2: "PF_UNSUPPORTED", 3: "PF_CUD
 SYMBOLS = ("pf_version", "pf_create", "pf_destroy", "pf_last_error", "pf_set_option",
            "pf_workspace_bytes", "pf_group_begin", "pf_phaseA_fwd", "pf_phaseB_fwd",
            "pf_phaseB_bwd", "pf_phaseC_bwd", "pf_group_end", "pf_offload", "pf_prefetch",
-           "pf_counter", "pf_profile_read")
+           "pf_counter", "pf_profile_read", "pf_group_mark_cached", "pf_segment_bwd")
 
 
 class PrefixFlowError(RuntimeError):
@@ -88,6 +88,10 @@ def lib() -> ctypes.CDLL:
     L.pf_phaseC_bwd.argtypes = [vp, T, T, vp, T, T, T, T, vp]
     L.pf_group_end.restype = i32
     L.pf_group_end.argtypes = [vp]
+    L.pf_group_mark_cached.restype = i32
+    L.pf_group_mark_cached.argtypes = [vp]
+    L.pf_segment_bwd.restype = i32
+    L.pf_segment_bwd.argtypes = [vp, i64, T, T, T, T, vp, T, T, vp, vp, T, T, vp]
     L.pf_offload.restype = i32
     L.pf_offload.argtypes = [vp, vp, vp, ctypes.c_size_t, vp]
     L.pf_prefetch.restype = i32
@@ -229,6 +233,16 @@ def pf_phaseC_bwd(grp: _Handle, Q1, O1, LSE1, dO1, dQ1, dK1, dV1, stream=None) -
     _check(lib().pf_phaseC_bwd(grp.ptr, as_tensor(Q1), as_tensor(O1), _ptr(LSE1), as_tensor(dO1),
                                as_tensor(dQ1), as_tensor(dK1), as_tensor(dV1), _stream(stream)),
            grp.ctx)
+
+
+def pf_group_mark_cached(grp: _Handle) -> None:
+    _check(lib().pf_group_mark_cached(grp.ptr), grp.ctx)
+
+
+def pf_segment_bwd(grp: _Handle, Q, K, V, O, LSE, dO, dQ, accK, accV, dK, dV, stream=None) -> None:
+    _check(lib().pf_segment_bwd(grp.ptr, int(Q.shape[0]), as_tensor(Q), as_tensor(K), as_tensor(V),
+                                as_tensor(O), _ptr(LSE), as_tensor(dO), as_tensor(dQ), _ptr(accK),
+                                _ptr(accV), as_tensor(dK), as_tensor(dV), _stream(stream)), grp.ctx)
 
 
 def pf_group_end(grp: _Handle) -> None:

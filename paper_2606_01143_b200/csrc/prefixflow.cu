@@ -39,6 +39,7 @@ struct pf_ctx {
     int bwd_pairs_per_item = 0;  // (seq, head) pairs per prefix-tile CTA; 0 = heuristic
     int bwd_heads_per_item = 0;  // query heads per causal-tile CTA; 0 = heuristic
     bool profile = false;
+    bool zero_accumulators = true;
     int64_t n_launches = 0;
     std::vector<ProfRec> prof;         // recorded, not yet read
     std::vector<cudaEvent_t> ev_pool;  // recycled events
@@ -480,6 +481,10 @@ pf_status pf_set_option(pf_ctx* ctx, const char* name, int64_t value) {
         (name[4] == 'p' ? ctx->bwd_pairs_per_item : ctx->bwd_heads_per_item) = int(value);
         return PF_OK;
     }
+    if (strcmp(name, "zero_accumulators") == 0) {
+        ctx->zero_accumulators = value != 0;
+        return PF_OK;
+    }
     if (strcmp(name, "profile") == 0) {
         ctx->profile = value != 0;
         return PF_OK;
@@ -553,9 +558,11 @@ pf_status pf_group_begin(pf_ctx* ctx, const pf_desc* desc, int64_t Lp, pf_tensor
     }
     if (!workspace || reinterpret_cast<uintptr_t>(workspace) % kAlign != 0)
         return fail(ctx, PF_WORKSPACE, "workspace is NULL or not 256-byte aligned");
-    if (workspace_bytes < pf_workspace_bytes(desc, Lp, 0))
-        return fail(ctx, PF_WORKSPACE, "workspace of %zu bytes < pf_workspace_bytes = %zu",
-                    workspace_bytes, pf_workspace_bytes(desc, Lp, 0));
+    // the capacity each call needs (Phase C: Lp rows; Phase B / segment: the wave's rows) is checked
+    // by that call; here only a workspace that could not serve any call is refused
+    if (workspace_bytes < pf_workspace_bytes(desc, 0, 0))
+        return fail(ctx, PF_WORKSPACE, "workspace of %zu bytes < the minimum pf_workspace_bytes(desc, 0, 0) = %zu",
+                    workspace_bytes, pf_workspace_bytes(desc, 0, 0));
     pf_group* g = new (std::nothrow) pf_group();
     if (!g) return fail(ctx, PF_CUDA_ERROR, "out of host memory");
     g->ctx = ctx;
@@ -570,7 +577,7 @@ pf_status pf_group_begin(pf_ctx* ctx, const pf_desc* desc, int64_t Lp, pf_tensor
     g->ws_bytes = workspace_bytes;
     g->ws_cap = ws_capacity(*desc, workspace_bytes);
     g->state = 0;
-    if (g->gK1 && Lp > 0) {
+    if (g->gK1 && Lp > 0 && ctx->zero_accumulators) {
         cudaStream_t s = static_cast<cudaStream_t>(stream);
         const size_t bytes = size_t(Lp) * Hkv * d * 4;
         cudaError_t e = cudaMemsetAsync(g->gK1, 0, bytes, s);
@@ -713,6 +720,51 @@ pf_status pf_phaseB_bwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens
         if (st) return st;
     }
     return PF_OK;
+}
+
+pf_status pf_group_mark_cached(pf_group* grp) {
+    if (!grp) return PF_INVALID_ARG;
+    if (grp->state != 0) return fail(grp->ctx, PF_STATE, "pf_group_mark_cached: the group already left its initial state");
+    grp->state = 1;
+    return PF_OK;
+}
+
+pf_status pf_segment_bwd(pf_group* grp, int64_t Ls, pf_tensor Q, pf_tensor K, pf_tensor V, pf_tensor O,
+                         const float* LSE, pf_tensor dO, pf_tensor dQ, float* accK, float* accV,
+                         pf_tensor dK, pf_tensor dV, void* stream) {
+    if (!grp) return PF_INVALID_ARG;
+    pf_ctx* ctx = grp->ctx;
+    if (grp->state != 1) return fail(ctx, PF_STATE, "pf_segment_bwd needs the cache marked valid (Phase A or pf_group_mark_cached)");
+    if (!grp->gK1 && grp->Lp > 0) return fail(ctx, PF_STATE, "pf_segment_bwd: the group was opened without gK1/gV1");
+    if (Ls < 0) return fail(ctx, PF_INVALID_ARG, "Ls < 0");
+    if (Ls == 0) return PF_OK;
+    const int Hq = grp->desc.n_q_heads, Hkv = grp->desc.n_kv_heads, d = grp->desc.head_dim;
+    pf_status st;
+    if ((st = check_tensor(ctx, "Q", Q, Ls, Hq, d))) return st;
+    if ((st = check_tensor(ctx, "K", K, Ls, Hkv, d))) return st;
+    if ((st = check_tensor(ctx, "V", V, Ls, Hkv, d))) return st;
+    if ((st = check_tensor(ctx, "O", O, Ls, Hq, d))) return st;
+    if ((st = check_tensor(ctx, "dO", dO, Ls, Hq, d))) return st;
+    if ((st = check_tensor(ctx, "dQ", dQ, Ls, Hq, d))) return st;
+    if ((st = check_tensor(ctx, "dK", dK, Ls, Hkv, d))) return st;
+    if ((st = check_tensor(ctx, "dV", dV, Ls, Hkv, d))) return st;
+    if (!LSE || !accK || !accV) return fail(ctx, PF_INVALID_ARG, "LSE / accK / accV is NULL");
+    if (reinterpret_cast<uintptr_t>(accK) % 16 != 0 || reinterpret_cast<uintptr_t>(accV) % 16 != 0)
+        return fail(ctx, PF_INVALID_ARG, "accK/accV must be 16-byte aligned");
+    if (align_up(Ls, 64) > grp->ws_cap)
+        return fail(ctx, PF_WORKSPACE, "workspace too small for a segment of %lld tokens", (long long)Ls);
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    const int64_t cu[2] = {0, Ls};
+    if (d == 64) {
+        st = launch_bwd<64>(grp, Q, grp->K1, grp->V1, grp->Lp, K, V, O, LSE, Ls, dO, grp->gK1, grp->gV1,
+                            accK, accV, dQ, 1, cu, 2, s);
+        if (!st) st = launch_convert_kv2<64>(grp, accK, dK, accV, dV, Ls, s);
+    } else {
+        st = launch_bwd<128>(grp, Q, grp->K1, grp->V1, grp->Lp, K, V, O, LSE, Ls, dO, grp->gK1, grp->gV1,
+                             accK, accV, dQ, 1, cu, 2, s);
+        if (!st) st = launch_convert_kv2<128>(grp, accK, dK, accV, dV, Ls, s);
+    }
+    return st;
 }
 
 pf_status pf_phaseC_bwd(pf_group* grp, pf_tensor Q1, pf_tensor O1, const float* LSE1,

@@ -398,3 +398,51 @@ def run_multilayer_step(ctx, layers, device="cuda", wave: int = 1, offload: bool
                 peak_step_bytes=max(peak_a, peak_b, torch.cuda.max_memory_allocated(dev)),
                 peak_phaseB_bytes=peak_b, resident_at_phaseB_start_bytes=base,
                 exposed_prefetch_ms=sum(a.elapsed_time(b) for a, b in exposed), outputs=outs)
+
+
+# --------------------------------------------------------------------------------------------------
+# Segment-by-segment training of one long sequence: causal
+# attention over [S_0 | S_1 | ... | S_m-1] computed one segment at a time.  Forward in order: segment k
+# attends to the cached K/V of segments < k (in place, rows [0, Lp_k) of the sequence's K/V) and
+# causally to itself.  Backward in reverse order: segment k's gradient reaches the earlier segments'
+# keys through the sequence-wide fp32 accumulator (gK/gV superposition, Proposition 3.1) and its
+# own key rows add onto what the later segments left there, rounded to bf16 once.
+# --------------------------------------------------------------------------------------------------
+def run_segmented_sequence(ctx, Q, K, V, dO, seg_lens: Sequence[int], stream=None) -> dict:
+    """Q, dO [L,Hq,d], K, V [L,Hkv,d] bf16 device tensors; returns O, LSE, dQ, dK, dV of the whole
+    sequence (identical, up to rounding order, to one full causal pass)."""
+    L, Hq, d = Q.shape
+    Hkv = K.shape[1]
+    assert sum(seg_lens) == L
+    dev = Q.device
+    desc = pf.make_desc(Hq, Hkv, d)
+    O = torch.empty_like(Q); dQ = torch.empty_like(Q)
+    dK = torch.empty_like(K); dV = torch.empty_like(V)
+    LSE = [torch.empty((Hq, n), dtype=torch.float32, device=dev) for n in seg_lens]
+    accK = torch.zeros((L, Hkv, d), dtype=torch.float32, device=dev)   # sequence-wide gK / gV
+    accV = torch.zeros((L, Hkv, d), dtype=torch.float32, device=dev)
+    ws = torch.empty(pf.pf_workspace_bytes(desc, 0, max(seg_lens)), dtype=torch.uint8, device=dev)
+    starts = [sum(seg_lens[:k]) for k in range(len(seg_lens))]
+    pf.pf_set_option(ctx, "zero_accumulators", 0)
+    try:
+        def open_group(k):
+            lo = starts[k]
+            g = pf.pf_group_begin(ctx, desc, lo, K[:lo], V[:lo], accK[:lo], accV[:lo], ws, stream)
+            pf.pf_group_mark_cached(g)
+            return g, slice(lo, lo + seg_lens[k])
+        for k in range(len(seg_lens)):                       # forward, in order
+            g, sl = open_group(k)
+            try:
+                pf.pf_phaseB_fwd(g, [0, seg_lens[k]], Q[sl], K[sl], V[sl], O[sl], LSE[k], stream)
+            finally:
+                pf.pf_group_end(g)
+        for k in range(len(seg_lens) - 1, -1, -1):           # backward, in reverse order
+            g, sl = open_group(k)
+            try:
+                pf.pf_segment_bwd(g, Q[sl], K[sl], V[sl], O[sl], LSE[k], dO[sl], dQ[sl],
+                                  accK[sl], accV[sl], dK[sl], dV[sl], stream)
+            finally:
+                pf.pf_group_end(g)
+    finally:
+        pf.pf_set_option(ctx, "zero_accumulators", 1)
+    return dict(O=O, LSE=torch.cat(LSE, 1), dQ=dQ, dK=dK, dV=dV)

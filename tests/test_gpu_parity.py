@@ -285,3 +285,24 @@ def test_multilayer_offload_pipeline(ctx, offload):
     if offload:
         base = schedule.run_multilayer_step(ctx, layers, wave=2, offload=False)
         assert r["peak_phaseB_bytes"] < base["peak_phaseB_bytes"]
+
+
+@pytest.mark.parametrize("Hq,Hkv,d,segs", [
+    (4, 2, 128, [130, 64, 200, 1, 127]),     # ragged segments, one of a single token
+    (7, 1, 64, [64, 64, 64]),                # d = 64, GQA 7:1, exact tiles
+    (2, 2, 128, [300]),                      # one segment = one full causal pass
+])
+def test_segment_by_segment_equals_full_causal_pass(ctx, Hq, Hkv, d, segs):
+    """a long sequence trained segment by segment, gK/gV accumulated into earlier
+    segments, equals full-sequence causal attention forward + backward (the oracle's definition)."""
+    L = sum(segs)
+    shape = inputs.small_case(Hq, Hkv, d, L, [], seed=61, dist="unit")
+    inp = inputs.make_group(shape)                            # Q1, K1, V1, dO1 = the whole sequence
+    from oracle import reference as oref
+    ref = oref.fullseq(oref.widen(inp.Q1), oref.widen(inp.K1), oref.widen(inp.V1), oref.widen(inp.dO1), 0)
+    dev = "cuda"
+    r = schedule.run_segmented_sequence(ctx, inp.Q1.to(dev), inp.K1.to(dev), inp.V1.to(dev),
+                                        inp.dO1.to(dev), segs)
+    torch.cuda.synchronize()
+    check("O", r["O"], ref["o"]); check("LSE", r["LSE"], ref["lse"], lse=True)
+    check("dQ", r["dQ"], ref["dq"]); check("dK", r["dK"], ref["dk"]); check("dV", r["dV"], ref["dv"])
