@@ -362,6 +362,10 @@ pf_status launch_bwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const
     int ppcP = ctx->bwd_pairs_per_item > 0 ? ctx->bwd_pairs_per_item
                                            : int(std::lround(target / std::fmax(1.0, avg_nqs)));
     ppcP = ppcP < 1 ? 1 : (ppcP > pairs ? pairs : ppcP);
+    if (ctx->bwd_pairs_per_item == 0 && pairs > 0) {   // even chunks: no tiny last item
+        const int chunks = (pairs + ppcP - 1) / ppcP;
+        ppcP = (pairs + chunks - 1) / chunks;
+    }
     int ppcC = ctx->bwd_heads_per_item > 0 ? ctx->bwd_heads_per_item
                                            : int(std::lround(target / std::fmax(1.0, avg_nqs)));
     const int capC = ctx->bwd_heads_per_item > 0 ? G : (G + 1) / 2;   // measured: G heads per causal item is too coarse
