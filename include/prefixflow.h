@@ -154,6 +154,15 @@ pf_status pf_phaseC_bwd(pf_group* grp, pf_tensor Q1, pf_tensor O1, const float* 
  *                          segments on entry) and dK, dV = bf16(accK), bf16(accV) on exit -- one rounding.
  * Run the segments in order for the forward and in reverse order for the backward. */
 pf_status pf_group_mark_cached(pf_group* grp);
+
+/* Tree-structured data ("each internal node of tree-structured RL data can carry its own
+ * K/V cache and gK/gV accumulator"): restrict the prefix that later pf_phaseB_fwd / pf_phaseB_bwd /
+ * pf_segment_bwd calls of this group see to n_ranges <= 8 ascending, non-overlapping row ranges
+ * [start, start+len) of the K1/V1 (and gK1/gV1) buffers -- the ancestors of the node being processed
+ * when all nodes of the tree are stored in one buffer in depth-first order.  Keys outside the ranges
+ * are invisible and receive no gradient.  n_ranges = 0 hides the whole prefix.  Host-side only. */
+pf_status pf_group_set_prefix_ranges(pf_group* grp, int32_t n_ranges, const int64_t* starts_host,
+                                     const int64_t* lens_host);
 pf_status pf_segment_bwd(pf_group* grp, int64_t Ls, pf_tensor Q, pf_tensor K, pf_tensor V, pf_tensor O,
                          const float* LSE, pf_tensor dO, pf_tensor dQ, float* accK, float* accV,
                          pf_tensor dK, pf_tensor dV, void* stream);

@@ -24,7 +24,8 @@ STATUS_NAMES = {0: "PF_OK", 1: "PF_INVALID_ARG", 2: "PF_UNSUPPORTED", 3: "PF_CUD
 SYMBOLS = ("pf_version", "pf_create", "pf_destroy", "pf_last_error", "pf_set_option",
            "pf_workspace_bytes", "pf_group_begin", "pf_phaseA_fwd", "pf_phaseB_fwd",
            "pf_phaseB_bwd", "pf_phaseC_bwd", "pf_group_end", "pf_offload", "pf_prefetch",
-           "pf_counter", "pf_profile_read", "pf_group_mark_cached", "pf_segment_bwd")
+           "pf_counter", "pf_profile_read", "pf_group_mark_cached", "pf_segment_bwd",
+           "pf_group_set_prefix_ranges")
 
 
 class PrefixFlowError(RuntimeError):
@@ -90,6 +91,8 @@ def lib() -> ctypes.CDLL:
     L.pf_group_end.argtypes = [vp]
     L.pf_group_mark_cached.restype = i32
     L.pf_group_mark_cached.argtypes = [vp]
+    L.pf_group_set_prefix_ranges.restype = i32
+    L.pf_group_set_prefix_ranges.argtypes = [vp, i32, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64)]
     L.pf_segment_bwd.restype = i32
     L.pf_segment_bwd.argtypes = [vp, i64, T, T, T, T, vp, T, T, vp, vp, T, T, vp]
     L.pf_offload.restype = i32
@@ -237,6 +240,14 @@ def pf_phaseC_bwd(grp: _Handle, Q1, O1, LSE1, dO1, dQ1, dK1, dV1, stream=None) -
 
 def pf_group_mark_cached(grp: _Handle) -> None:
     _check(lib().pf_group_mark_cached(grp.ptr), grp.ctx)
+
+
+def pf_group_set_prefix_ranges(grp: _Handle, ranges: Sequence[Sequence[int]]) -> None:
+    """ranges: [(start, len), ...] ascending rows of the K1/V1 buffer visible as the prefix."""
+    n = len(ranges)
+    starts = (ctypes.c_int64 * max(1, n))(*[int(r[0]) for r in ranges])
+    lens = (ctypes.c_int64 * max(1, n))(*[int(r[1]) for r in ranges])
+    _check(lib().pf_group_set_prefix_ranges(grp.ptr, n, starts, lens), grp.ctx)
 
 
 def pf_segment_bwd(grp: _Handle, Q, K, V, O, LSE, dO, dQ, accK, accV, dK, dV, stream=None) -> None:

@@ -38,9 +38,9 @@ struct BwdParams {
     const float* lse2;             // [Hq, stat_stride] LSE * log2(e) at padded positions; +inf in pads
     const float* delta;            // [Hq, stat_stride] rowsum(dO o O); 0 in pads
     int64_t stat_stride;
-    int Lp;
+    PrefixRanges pre;              // visible ranges of the prefix source
     int Hq, Hkv, G;
-    int nPT;                       // ceil(Lp / 128)
+    int nPT;                       // 128-row tiles of the prefix ranges = pre.tile0[pre.n]
     int nQS;                       // total query sub-tiles = seq.pqs[seq.n]
     int chunksP, ppcP;             // prefix items: the n*G (seq, head) pairs in chunks of ppcP
     int chunksC, ppcC;             // causal items: the G heads of the sequence in chunks of ppcC
@@ -147,7 +147,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     // ---- item decode: prefix-source items first (heaviest), then the causal key tiles ----
     int item = blockIdx.x;
     const bool pre = item < p.nItemsP;
-    int kt, g, pair_lo, pair_hi, qs_lo, kvrow0;
+    int kt, g, pair_lo, pair_hi, qs_lo, kvrow0, kvalid = 128;   // kvalid: rows of the tile inside its prefix range
     if (pre) {
         // chunk-major order: the CTAs that run at the same time walk the SAME (sequence, head) pairs
         // over different key tiles, so their Q/dO tiles and the dQ^T tiles they reduce into stay
@@ -159,7 +159,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         pair_lo = (item / per) * p.ppcP;
         pair_hi = min(p.seq.n * p.G, pair_lo + p.ppcP);
         qs_lo = 0;
-        kvrow0 = kt * 128;
+        p.pre.locate(kt, kvrow0, kvalid);
     } else {
         item -= p.nItemsP;
         const int per = p.Hkv * p.chunksC;
@@ -321,8 +321,9 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     tmem_ld_16x256b_x4(tDP_w + b * 64 + (uint32_t(blk * 16) << 16), dp[blk]);
                 }
                 tmem_wait_ld();
-                // causal source: query t sees key kj iff t >= kj; only diagonal sub-tiles need it
-                const bool diag = !pre && iter.qs * 64 < kt * 128 + 128;
+                // causal source: query t sees key kj iff t >= kj; only diagonal sub-tiles need it.
+                // prefix source: rows past the end of the tile's range (another node's keys) see nothing.
+                const bool diag = pre ? kvalid < 128 : iter.qs * 64 < kt * 128 + 128;
                 const int col0 = iter.qs * 64 + w * 32 + 2 * lq;  // query (within its sequence) of r = 0, e = 0
 #pragma unroll
                 for (int blk = 0; blk < 2; ++blk) {
@@ -330,7 +331,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 #pragma unroll
                     for (int hf = 0; hf < 2; ++hf) {
                         const int row = (warp & 3) * 32 + blk * 16 + hf * 8 + lr;   // key row in tile
-                        const int kj = kt * 128 + row;
+                        const int kj = pre ? (row >= kvalid ? 0x7fffffff : -1) : kt * 128 + row;
 #pragma unroll
                         for (int r = 0; r < 4; ++r) {
                             const int i = r * 4 + hf * 2;

@@ -38,7 +38,7 @@ struct FwdParams {
     int64_t o_stride_tok, o_stride_head;  // elements
     float* LSE;                           // [Hq, lse_stride], column = packed token row
     int64_t lse_stride;
-    int Lp;        // prefix-source keys (0: none)
+    PrefixRanges pre;  // visible ranges of the prefix source (n = 0: none)
     int Hq, Hkv, G;
     float scale_log2;  // sigma * log2(e)
     SeqTable seq;
@@ -111,7 +111,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
     const int tok0 = p.seq.cu[sq], Ls = p.seq.cu[sq + 1] - tok0;
     const int idx = nRB * p.G - 1 - (int(blockIdx.x) - base);
     const int rb = idx / p.G, h = g * p.G + idx % p.G;
-    const int nP = (p.Lp + 127) >> 7;
+    const int nP = p.pre.n > 0 ? p.pre.tile0[p.pre.n] : 0;
     const int n_iter = nP + rb + 1;
 
     if (tid == 0) {
@@ -145,7 +145,8 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
                 const int st = it % C::KS;
                 const uint32_t ph = (it / C::KS) & 1;
                 const bool pre = it < nP;
-                const int row0 = pre ? it * 128 : tok0 + (it - nP) * 128;
+                int row0 = tok0 + (it - nP) * 128, valid_rows;
+                if (pre) p.pre.locate(it, row0, valid_rows);
                 mbar_wait(&bar_Ke[st], ph ^ 1);
                 mbar_arrive_expect_tx(&bar_Kf[st], C::TILE);
                 for (int k = 0; k < C::NSUB; ++k)
@@ -243,7 +244,12 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
             tmem_ld32(tS, x);
             tmem_wait_ld();
             // visible keys of this tile for this row, relative to this quarter's first column
-            const int limit = (it < nP ? p.Lp - it * 128 : t - (it - nP) * 128 + 1) - qd * 32;
+            int limit = t - (it - nP) * 128 + 1;
+            if (it < nP) {
+                int row0;
+                p.pre.locate(it, row0, limit);
+            }
+            limit -= qd * 32;
             if (limit < 32) {                    // ragged prefix tail or causal diagonal
 #pragma unroll
                 for (int j = 0; j < 32; ++j)

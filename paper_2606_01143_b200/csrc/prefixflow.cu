@@ -57,6 +57,7 @@ struct pf_group {
     uint8_t* ws;
     size_t ws_bytes;
     int64_t ws_cap;  // padded token positions the workspace holds (multiple of 64)
+    pf::PrefixRanges pre;  // visible ranges of the prefix source (default: [0, Lp))
     int state;  // 0 begun, 1 A done, 2 C done
 };
 
@@ -226,6 +227,17 @@ pf_status set_attrs() {
     return PF_OK;
 }
 
+pf::PrefixRanges whole_prefix(int64_t Lp) {
+    pf::PrefixRanges r;
+    memset(&r, 0, sizeof(r));
+    if (Lp > 0) {
+        r.n = 1;
+        r.len[0] = int(Lp);
+        r.tile0[1] = int((Lp + 127) / 128);
+    }
+    return r;
+}
+
 // Sequence table of one launch from host offsets cu[0..n] (cu[0] = 0, n <= kMaxSeqs)
 pf::SeqTable make_seq_table(int n, const int64_t* cu) {
     pf::SeqTable t;
@@ -270,7 +282,7 @@ pf_status launch_fwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const
     p.o_stride_head = O.stride_head;
     p.LSE = LSE;
     p.lse_stride = lse_stride;
-    p.Lp = int(Lp);
+    p.pre = Lp > 0 ? g->pre : whole_prefix(0);
     p.Hq = Hq;
     p.Hkv = Hkv;
     p.G = Hq / Hkv;
@@ -344,9 +356,9 @@ pf_status launch_bwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const
     pf::BwdParams p;
     p.dQacc = dqacc;
     p.lse2 = lse2; p.delta = delta; p.stat_stride = w.stat_stride;
-    p.Lp = int(Lp);
+    p.pre = Lp > 0 ? g->pre : whole_prefix(0);
     p.Hq = Hq; p.Hkv = Hkv; p.G = G;
-    p.nPT = int((Lp + 127) / 128);
+    p.nPT = p.pre.n > 0 ? p.pre.tile0[p.pre.n] : 0;
     p.nQS = nQS;
     p.seq = seq;
     // ---- item sizing: aim at >= ~6 items per SM, each long enough to amortise its prologue
@@ -580,6 +592,7 @@ pf_status pf_group_begin(pf_ctx* ctx, const pf_desc* desc, int64_t Lp, pf_tensor
     g->ws = static_cast<uint8_t*>(workspace);
     g->ws_bytes = workspace_bytes;
     g->ws_cap = ws_capacity(*desc, workspace_bytes);
+    g->pre = whole_prefix(Lp);
     g->state = 0;
     if (g->gK1 && Lp > 0 && ctx->zero_accumulators) {
         cudaStream_t s = static_cast<cudaStream_t>(stream);
@@ -723,6 +736,31 @@ pf_status pf_phaseB_bwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens
         }
         if (st) return st;
     }
+    return PF_OK;
+}
+
+pf_status pf_group_set_prefix_ranges(pf_group* grp, int32_t n_ranges, const int64_t* starts_host,
+                                     const int64_t* lens_host) {
+    if (!grp) return PF_INVALID_ARG;
+    pf_ctx* ctx = grp->ctx;
+    if (n_ranges < 0 || n_ranges > pf::kMaxRanges)
+        return fail(ctx, PF_UNSUPPORTED, "n_ranges=%d not in [0, %d]", n_ranges, pf::kMaxRanges);
+    if (n_ranges > 0 && (!starts_host || !lens_host)) return fail(ctx, PF_INVALID_ARG, "ranges are NULL");
+    pf::PrefixRanges r;
+    memset(&r, 0, sizeof(r));
+    int64_t end = 0;
+    for (int i = 0; i < n_ranges; ++i) {
+        if (lens_host[i] <= 0) continue;   // empty ranges are dropped
+        if (starts_host[i] < end || starts_host[i] + lens_host[i] > grp->Lp)
+            return fail(ctx, PF_INVALID_ARG, "prefix range %d = [%lld, +%lld) is out of [0, Lp) or not ascending",
+                        i, (long long)starts_host[i], (long long)lens_host[i]);
+        r.start[r.n] = int(starts_host[i]);
+        r.len[r.n] = int(lens_host[i]);
+        r.tile0[r.n + 1] = r.tile0[r.n] + int((lens_host[i] + 127) / 128);
+        end = starts_host[i] + lens_host[i];
+        ++r.n;
+    }
+    grp->pre = r;
     return PF_OK;
 }
 

@@ -446,3 +446,81 @@ def run_segmented_sequence(ctx, Q, K, V, dO, seg_lens: Sequence[int], stream=Non
     finally:
         pf.pf_set_option(ctx, "zero_accumulators", 1)
     return dict(O=O, LSE=torch.cat(LSE, 1), dQ=dQ, dK=dK, dV=dV)
+
+
+# --------------------------------------------------------------------------------------------------
+# Tree-structured data: all nodes of a prefix tree stored in ONE
+# [L, H, d] buffer in depth-first order; a node attends to its ancestors (row ranges of the buffer
+# before it, `pf_group_set_prefix_ranges`) and causally to itself.  Forward in DFS order; backward in
+# reverse DFS order, every node adding into its ancestors' rows of the tree-wide fp32 gK/gV
+# accumulator and finishing its own rows (children first, so all contributions have arrived).
+# --------------------------------------------------------------------------------------------------
+def tree_ranges(nodes: Sequence[Sequence[int]]):
+    """nodes[i] = (parent index or -1, length), in DFS order.  Returns (starts, per-node ancestor
+    ranges [(start, len), ...] with adjacent ranges merged)."""
+    starts, out = [], []
+    pos = 0
+    for parent, n in nodes:
+        starts.append(pos)
+        pos += n
+    for i, (parent, n) in enumerate(nodes):
+        path = []
+        a = parent
+        while a >= 0:
+            path.append(a)
+            a = nodes[a][0]
+        rs = []
+        for a in reversed(path):
+            if nodes[a][1] == 0:
+                continue
+            if rs and rs[-1][0] + rs[-1][1] == starts[a]:
+                rs[-1] = (rs[-1][0], rs[-1][1] + nodes[a][1])
+            else:
+                rs.append((starts[a], nodes[a][1]))
+        out.append(rs)
+    return starts, out
+
+
+def run_tree(ctx, Q, K, V, dO, nodes: Sequence[Sequence[int]], stream=None) -> dict:
+    """Attention forward + backward over a prefix tree (see above); returns O, LSE (per node), dQ, dK, dV."""
+    L, Hq, d = Q.shape
+    Hkv = K.shape[1]
+    lens = [n for _, n in nodes]
+    assert sum(lens) == L
+    dev = Q.device
+    desc = pf.make_desc(Hq, Hkv, d)
+    starts, ranges = tree_ranges(nodes)
+    O = torch.empty_like(Q); dQ = torch.empty_like(Q)
+    dK = torch.empty_like(K); dV = torch.empty_like(V)
+    LSE = [torch.empty((Hq, n), dtype=torch.float32, device=dev) for n in lens]
+    accK = torch.zeros((L, Hkv, d), dtype=torch.float32, device=dev)   # tree-wide gK / gV
+    accV = torch.zeros((L, Hkv, d), dtype=torch.float32, device=dev)
+    ws = torch.empty(pf.pf_workspace_bytes(desc, 0, max(lens)), dtype=torch.uint8, device=dev)
+    pf.pf_set_option(ctx, "zero_accumulators", 0)
+    try:
+        def open_group(i):
+            lo = starts[i]
+            g = pf.pf_group_begin(ctx, desc, lo, K[:lo], V[:lo], accK[:lo], accV[:lo], ws, stream)
+            pf.pf_group_set_prefix_ranges(g, ranges[i])
+            pf.pf_group_mark_cached(g)
+            return g, slice(lo, lo + lens[i])
+        for i in range(len(nodes)):
+            if lens[i] == 0:
+                continue
+            g, sl = open_group(i)
+            try:
+                pf.pf_phaseB_fwd(g, [0, lens[i]], Q[sl], K[sl], V[sl], O[sl], LSE[i], stream)
+            finally:
+                pf.pf_group_end(g)
+        for i in range(len(nodes) - 1, -1, -1):
+            if lens[i] == 0:
+                continue
+            g, sl = open_group(i)
+            try:
+                pf.pf_segment_bwd(g, Q[sl], K[sl], V[sl], O[sl], LSE[i], dO[sl], dQ[sl],
+                                  accK[sl], accV[sl], dK[sl], dV[sl], stream)
+            finally:
+                pf.pf_group_end(g)
+    finally:
+        pf.pf_set_option(ctx, "zero_accumulators", 1)
+    return dict(O=O, LSE=LSE, dQ=dQ, dK=dK, dV=dV, starts=starts)

@@ -306,3 +306,46 @@ def test_segment_by_segment_equals_full_causal_pass(ctx, Hq, Hkv, d, segs):
     torch.cuda.synchronize()
     check("O", r["O"], ref["o"]); check("LSE", r["LSE"], ref["lse"], lse=True)
     check("dQ", r["dQ"], ref["dq"]); check("dK", r["dK"], ref["dk"]); check("dV", r["dV"], ref["dv"])
+
+
+def _tree_oracle(inp, nodes):
+    """Every root-to-leaf path is one full causal sequence (the oracle's definition); a node shared
+    by several leaves carries 1/#leaves of its adjoint in each of them (reading 1)."""
+    from oracle import reference as oref
+    q, k, v, dO = (oref.widen(x) for x in (inp.Q1, inp.K1, inp.V1, inp.dO1))
+    starts, _ = schedule.tree_ranges(nodes)
+    children = [[j for j, (p, _) in enumerate(nodes) if p == i] for i in range(len(nodes))]
+    leaves = [i for i in range(len(nodes)) if not children[i]]
+    def path(i):
+        out = []
+        while i >= 0:
+            out.append(i); i = nodes[i][0]
+        return out[::-1]
+    nleaf = [sum(1 for l in leaves if i in path(l)) for i in range(len(nodes))]
+    L = q.shape[0]
+    ref = dict(o=np.zeros_like(q), lse=np.zeros((q.shape[1], L)), dq=np.zeros_like(q),
+               dk=np.zeros_like(k), dv=np.zeros_like(v))
+    for l in leaves:
+        rows = np.concatenate([np.arange(starts[i], starts[i] + nodes[i][1]) for i in path(l)])
+        w = np.concatenate([np.full(nodes[i][1], 1.0 / nleaf[i]) for i in path(l)])
+        r = oref.fullseq(q[rows], k[rows], v[rows], dO[rows] * w[:, None, None], 0)
+        ref["o"][rows] = r["o"]; ref["lse"][:, rows] = r["lse"]
+        ref["dq"][rows] += r["dq"]; ref["dk"][rows] += r["dk"]; ref["dv"][rows] += r["dv"]
+    return ref
+
+
+@pytest.mark.parametrize("Hq,Hkv,d,nodes", [
+    # root -> {A -> {a1, a2}, B -> {b1}} with ragged lengths (ranges not tile aligned)
+    (4, 2, 128, [(-1, 200), (0, 70), (1, 130), (1, 64), (0, 129), (4, 90)]),
+    # a chain (= segment-by-segment) and a bushy root, d = 64
+    (2, 1, 64, [(-1, 128), (0, 65), (0, 1), (0, 127), (3, 64)]),
+])
+def test_tree_structured_prefixes(ctx, Hq, Hkv, d, nodes):
+    L = sum(n for _, n in nodes)
+    inp = inputs.make_group(inputs.small_case(Hq, Hkv, d, L, [], seed=71, dist="unit"))
+    ref = _tree_oracle(inp, nodes)
+    dev = "cuda"
+    r = schedule.run_tree(ctx, inp.Q1.to(dev), inp.K1.to(dev), inp.V1.to(dev), inp.dO1.to(dev), nodes)
+    torch.cuda.synchronize()
+    check("O", r["O"], ref["o"]); check("LSE", torch.cat(r["LSE"], 1), ref["lse"], lse=True)
+    check("dQ", r["dQ"], ref["dq"]); check("dK", r["dK"], ref["dk"]); check("dV", r["dV"], ref["dv"])
