@@ -18,7 +18,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 def run(config: str, steps: int) -> dict:
     cmd = [sys.executable, os.path.join(ROOT, "bench.py"), "--config", config, "--steps", str(steps),
-           "--no-cpu", "--no-e2e", "--no-wave1"]
+           "--no-cpu", "--no-e2e", "--no-wave1", "--no-offload"]
     out = subprocess.run(cmd, capture_output=True, text=True, check=True).stdout.strip().splitlines()
     return json.loads(out[-1])
 
