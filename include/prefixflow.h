@@ -25,7 +25,13 @@
  *   - gK1 / gV1 are fp32, contiguous [Lp, Hkv, d], borrowed for the lifetime of the group;
  *   - head_dim in {64, 128}; softmax_scale 0 means 1/sqrt(head_dim);
  *   - functions return a pf_status; nothing throws or aborts across this boundary; validation
- *     happens before any launch; Ls = 0 and Lp = 0 are legal.
+ *     happens before any launch; Ls = 0 and Lp = 0 are legal;
+ *   - every element of the tensors a call reads must be FINITE, including rows of K1/V1 that a
+ *     prefix-range restriction (pf_group_set_prefix_ranges) hides and rows of a packed wave that
+ *     belong to another sequence: masked keys get probability exactly 0 but their values still
+ *     pass through the tensor cores (0 x NaN = NaN);
+ *   - a context is bound to one CUDA device, which must be the current device of the calling
+ *     thread for every call that takes the context or one of its groups (PF_STATE otherwise).
  */
 #ifndef PREFIXFLOW_H_
 #define PREFIXFLOW_H_
@@ -65,7 +71,8 @@ typedef struct {
 
 int32_t pf_version(void);
 
-/* Create / destroy a context bound to CUDA device `device` (host-side state only). */
+/* Create / destroy a context bound to CUDA device `device` (host-side state only; the caller's
+ * current device is left as it was). */
 pf_status pf_create(pf_ctx** out, int32_t device);
 pf_status pf_destroy(pf_ctx* ctx);
 /* Message of the last failing call on this context (valid until the next call). */
@@ -86,8 +93,12 @@ pf_status pf_set_option(pf_ctx* ctx, const char* name, int64_t value);
  *                      with a pair of CUDA events on the launch stream; read with pf_profile_read.
  *                      Used by bench.py for the roofline of the dominant kernel.  0 = off. */
 
-/* Number of kernels this context has launched so far ("kernel_launches"), or -1 for an unknown
- * counter name.  Host-side bookkeeping only. */
+/* Counters; -1 for an unknown name.
+ *   "kernel_launches"  : kernels this context has launched so far (host-side bookkeeping).
+ *   "fwd_rescale_rows" : process-wide count of (query row, KV tile) events in which the forward kernel
+ *                        re-based the running softmax maximum after the row's first tile (the lazy
+ *                        rescale of the O accumulator).  Debug evidence for the tests; reading it
+ *                        synchronises the device. */
 int64_t pf_counter(const pf_ctx* ctx, const char* name);
 
 /* Profiling read-out (needs option "profile" = 1).  kind: the call that launched the attention
@@ -120,19 +131,19 @@ pf_status pf_phaseA_fwd(pf_group* grp, pf_tensor Q1, pf_tensor O1, float* LSE1, 
  * the token axis (cu_seqlens_host[n_seqs+1], cu[0] = 0; the usual case is n_seqs = 1), the
  * queries of suffix i attend to all Lp cached prefix keys and causally to the keys of suffix i
  * only.  Q2,O2: [sumLs,Hq,d]; K2,V2: [sumLs,Hkv,d]; LSE2: [Hq,sumLs].  K1/V1 are read in place
- * (no concatenation copy).  cu_seqlens_dev is reserved (may be NULL). */
-pf_status pf_phaseB_fwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens_dev,
-                        const int32_t* cu_seqlens_host, pf_tensor Q2, pf_tensor K2, pf_tensor V2,
-                        pf_tensor O2, float* LSE2, void* stream);
+ * (no concatenation copy).  The sequence offsets are a HOST array: the launch
+ * geometry depends on them, and the kernels receive them by value (no device copy is read). */
+pf_status pf_phaseB_fwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens_host,
+                        pf_tensor Q2, pf_tensor K2, pf_tensor V2, pf_tensor O2, float* LSE2,
+                        void* stream);
 
 /* Phase B backward: dQ2 [sumLs,Hq,d], dK2, dV2 [sumLs,Hkv,d] bf16 of the
  * suffix tokens, and   gK1 += sigma dS21^T Q2,  gV1 += P21^T dO2   (summed over the G query heads
  * of each KV head; fp32; the accumulators persist across calls).  Calls of one
  * group must be stream-ordered or on streams the caller orders. */
-pf_status pf_phaseB_bwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens_dev,
-                        const int32_t* cu_seqlens_host, pf_tensor Q2, pf_tensor K2, pf_tensor V2,
-                        pf_tensor O2, const float* LSE2, pf_tensor dO2, pf_tensor dQ2,
-                        pf_tensor dK2, pf_tensor dV2, void* stream);
+pf_status pf_phaseB_bwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens_host,
+                        pf_tensor Q2, pf_tensor K2, pf_tensor V2, pf_tensor O2, const float* LSE2,
+                        pf_tensor dO2, pf_tensor dQ2, pf_tensor dK2, pf_tensor dV2, void* stream);
 
 /* Phase C: causal backward over the prefix; dQ1 [Lp,Hq,d] and
  * dK1 = bf16(own-prefix term + gK1), dV1 = bf16(own-prefix term + gV1), the sum taken in fp32

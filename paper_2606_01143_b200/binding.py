@@ -82,9 +82,9 @@ def lib() -> ctypes.CDLL:
     L.pf_phaseA_fwd.restype = i32
     L.pf_phaseA_fwd.argtypes = [vp, T, T, vp, vp]
     L.pf_phaseB_fwd.restype = i32
-    L.pf_phaseB_fwd.argtypes = [vp, i32, pi32, pi32, T, T, T, T, vp, vp]
+    L.pf_phaseB_fwd.argtypes = [vp, i32, pi32, T, T, T, T, vp, vp]
     L.pf_phaseB_bwd.restype = i32
-    L.pf_phaseB_bwd.argtypes = [vp, i32, pi32, pi32, T, T, T, T, vp, T, T, T, T, vp]
+    L.pf_phaseB_bwd.argtypes = [vp, i32, pi32, T, T, T, T, vp, T, T, T, T, vp]
     L.pf_phaseC_bwd.restype = i32
     L.pf_phaseC_bwd.argtypes = [vp, T, T, vp, T, T, T, T, vp]
     L.pf_group_end.restype = i32
@@ -120,6 +120,35 @@ def as_tensor(t: Optional[torch.Tensor], dtype=torch.bfloat16) -> pf_tensor:
 
 def _ptr(t: Optional[torch.Tensor]):
     return None if t is None or t.numel() == 0 else t.data_ptr()
+
+
+def _stat(t: Optional[torch.Tensor], Hq: int, L: int, name: str):
+    """fp32 [Hq, L] statistics tensor (LSE) -> raw pointer.  The C side assumes row stride = L, so a
+    column slice of a wider tensor (non-contiguous) must be refused here, not written out of bounds."""
+    if L == 0:
+        return None
+    if (t is None or t.dtype != torch.float32 or tuple(t.shape) != (Hq, L) or not t.is_contiguous()
+            or not t.is_cuda):
+        raise PrefixFlowError(PF_INVALID_ARG, f"{name} must be a contiguous CUDA float32 tensor of shape "
+                              f"({Hq}, {L}), got {None if t is None else (tuple(t.shape), t.dtype, t.is_contiguous())}")
+    return t.data_ptr()
+
+
+def _acc(t: torch.Tensor, like: torch.Tensor, name: str):
+    """fp32 accumulator rows [L, Hkv, d], contiguous, same shape as the bf16 tensor `like`."""
+    if (t.dtype != torch.float32 or tuple(t.shape) != tuple(like.shape) or not t.is_contiguous()
+            or not t.is_cuda):
+        raise PrefixFlowError(PF_INVALID_ARG, f"{name} must be a contiguous CUDA float32 tensor of shape "
+                              f"{tuple(like.shape)}, got {tuple(t.shape)} {t.dtype}")
+    return _ptr(t)
+
+
+def _flat(t: torch.Tensor, name: str, cuda: bool):
+    """Contiguous buffer for a raw byte copy (pf_offload / pf_prefetch)."""
+    if not t.is_contiguous() or t.is_cuda != cuda or (not cuda and not t.is_pinned()):
+        raise PrefixFlowError(PF_INVALID_ARG, f"{name} must be a contiguous "
+                              f"{'CUDA' if cuda else 'pinned host'} tensor")
+    return _ptr(t)
 
 
 def _stream(stream) -> Optional[int]:
@@ -209,31 +238,30 @@ def pf_group_begin(ctx: _Handle, desc: pf_desc, Lp: int, K1, V1, gK1, gV1, works
 
 
 def pf_phaseA_fwd(grp: _Handle, Q1, O1, LSE1, stream=None) -> None:
-    _check(lib().pf_phaseA_fwd(grp.ptr, as_tensor(Q1), as_tensor(O1), _ptr(LSE1), _stream(stream)),
-           grp.ctx)
+    _check(lib().pf_phaseA_fwd(grp.ptr, as_tensor(Q1), as_tensor(O1),
+                               _stat(LSE1, Q1.shape[1], Q1.shape[0], "LSE1"), _stream(stream)), grp.ctx)
 
 
 def pf_phaseB_fwd(grp: _Handle, cu_seqlens_host: Sequence[int], Q2, K2, V2, O2, LSE2,
-                  stream=None, cu_seqlens_dev: Optional[torch.Tensor] = None) -> None:
+                  stream=None) -> None:
     cu = _cu(cu_seqlens_host)
-    _check(lib().pf_phaseB_fwd(grp.ptr, len(cu_seqlens_host) - 1,
-                               ctypes.cast(_ptr(cu_seqlens_dev), ctypes.POINTER(ctypes.c_int32)), cu,
+    _check(lib().pf_phaseB_fwd(grp.ptr, len(cu_seqlens_host) - 1, cu,
                                as_tensor(Q2), as_tensor(K2), as_tensor(V2), as_tensor(O2),
-                               _ptr(LSE2), _stream(stream)), grp.ctx)
+                               _stat(LSE2, Q2.shape[1], Q2.shape[0], "LSE2"), _stream(stream)), grp.ctx)
 
 
 def pf_phaseB_bwd(grp: _Handle, cu_seqlens_host: Sequence[int], Q2, K2, V2, O2, LSE2, dO2, dQ2, dK2,
-                  dV2, stream=None, cu_seqlens_dev: Optional[torch.Tensor] = None) -> None:
+                  dV2, stream=None) -> None:
     cu = _cu(cu_seqlens_host)
-    _check(lib().pf_phaseB_bwd(grp.ptr, len(cu_seqlens_host) - 1,
-                               ctypes.cast(_ptr(cu_seqlens_dev), ctypes.POINTER(ctypes.c_int32)), cu,
+    _check(lib().pf_phaseB_bwd(grp.ptr, len(cu_seqlens_host) - 1, cu,
                                as_tensor(Q2), as_tensor(K2), as_tensor(V2), as_tensor(O2),
-                               _ptr(LSE2), as_tensor(dO2), as_tensor(dQ2), as_tensor(dK2),
-                               as_tensor(dV2), _stream(stream)), grp.ctx)
+                               _stat(LSE2, Q2.shape[1], Q2.shape[0], "LSE2"), as_tensor(dO2),
+                               as_tensor(dQ2), as_tensor(dK2), as_tensor(dV2), _stream(stream)), grp.ctx)
 
 
 def pf_phaseC_bwd(grp: _Handle, Q1, O1, LSE1, dO1, dQ1, dK1, dV1, stream=None) -> None:
-    _check(lib().pf_phaseC_bwd(grp.ptr, as_tensor(Q1), as_tensor(O1), _ptr(LSE1), as_tensor(dO1),
+    _check(lib().pf_phaseC_bwd(grp.ptr, as_tensor(Q1), as_tensor(O1),
+                               _stat(LSE1, Q1.shape[1], Q1.shape[0], "LSE1"), as_tensor(dO1),
                                as_tensor(dQ1), as_tensor(dK1), as_tensor(dV1), _stream(stream)),
            grp.ctx)
 
@@ -252,8 +280,9 @@ def pf_group_set_prefix_ranges(grp: _Handle, ranges: Sequence[Sequence[int]]) ->
 
 def pf_segment_bwd(grp: _Handle, Q, K, V, O, LSE, dO, dQ, accK, accV, dK, dV, stream=None) -> None:
     _check(lib().pf_segment_bwd(grp.ptr, int(Q.shape[0]), as_tensor(Q), as_tensor(K), as_tensor(V),
-                                as_tensor(O), _ptr(LSE), as_tensor(dO), as_tensor(dQ), _ptr(accK),
-                                _ptr(accV), as_tensor(dK), as_tensor(dV), _stream(stream)), grp.ctx)
+                                as_tensor(O), _stat(LSE, Q.shape[1], Q.shape[0], "LSE"), as_tensor(dO),
+                                as_tensor(dQ), _acc(accK, K, "accK"), _acc(accV, V, "accV"),
+                                as_tensor(dK), as_tensor(dV), _stream(stream)), grp.ctx)
 
 
 def pf_group_end(grp: _Handle) -> None:
@@ -263,9 +292,15 @@ def pf_group_end(grp: _Handle) -> None:
 
 def pf_offload(ctx: _Handle, src_dev: torch.Tensor, dst_pinned_host: torch.Tensor, stream) -> None:
     nbytes = src_dev.numel() * src_dev.element_size()
-    _check(lib().pf_offload(ctx.ptr, _ptr(src_dev), _ptr(dst_pinned_host), nbytes, _stream(stream)), ctx)
+    if dst_pinned_host.numel() * dst_pinned_host.element_size() < nbytes:
+        raise PrefixFlowError(PF_INVALID_ARG, "pf_offload: destination smaller than source")
+    _check(lib().pf_offload(ctx.ptr, _flat(src_dev, "src_dev", True),
+                            _flat(dst_pinned_host, "dst_pinned_host", False), nbytes, _stream(stream)), ctx)
 
 
 def pf_prefetch(ctx: _Handle, src_pinned_host: torch.Tensor, dst_dev: torch.Tensor, stream) -> None:
     nbytes = dst_dev.numel() * dst_dev.element_size()
-    _check(lib().pf_prefetch(ctx.ptr, _ptr(src_pinned_host), _ptr(dst_dev), nbytes, _stream(stream)), ctx)
+    if src_pinned_host.numel() * src_pinned_host.element_size() < nbytes:
+        raise PrefixFlowError(PF_INVALID_ARG, "pf_prefetch: source smaller than destination")
+    _check(lib().pf_prefetch(ctx.ptr, _flat(src_pinned_host, "src_pinned_host", False),
+                             _flat(dst_dev, "dst_dev", True), nbytes, _stream(stream)), ctx)

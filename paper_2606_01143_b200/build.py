@@ -38,8 +38,7 @@ def build_library(force: bool = False, verbose: bool = False) -> str:
     if not force and not needs_build():
         return SO_PATH
     nvcc = os.environ.get("NVCC", "nvcc")
-    extra = os.environ.get("PF_NVCC_EXTRA", "").split()   # e.g. -DPF_FWD_POLY16=4 for tuning sweeps
-    cmd = [nvcc, *NVCC_FLAGS, *extra, "-I", INCLUDE, "-o", SO_PATH, os.path.join(CSRC, "prefixflow.cu")]
+    cmd = [nvcc, *NVCC_FLAGS, "-I", INCLUDE, "-o", SO_PATH, os.path.join(CSRC, "prefixflow.cu")]
     if verbose:
         cmd[1:1] = ["-Xptxas", "-v"]
         print(" ".join(cmd), file=sys.stderr)

@@ -2,7 +2,7 @@
 //   bwd_preprocess : delta[h,t] = <dO[t,h], O[t,h]>,  lse2 = LSE * log2(e),
 //                    every sequence padded to a multiple of 64 rows (+inf / 0) for the tile loads
 //   dq_finish      : fp32 dQ^T tile workspace of the backward -> bf16 dQ rows
-//   acc_to_bf16    : fp32 staging [L,H,D] (contiguous) * scale -> bf16 strided output
+//   acc2_to_bf16   : two fp32 accumulators [L,H,D] (contiguous: dK and dV) -> bf16 strided outputs
 // Each thread moves 16 bytes of bf16 (8 elements); rows are coalesced along d.
 #pragma once
 #include <cuda_runtime.h>
@@ -118,32 +118,6 @@ acc2_to_bf16_kernel(const float* __restrict__ src0, __nv_bfloat16* __restrict__ 
     __nv_bfloat162 p1 = __floats2bfloat162_rn(a.z, a.w);
     __nv_bfloat162 p2 = __floats2bfloat162_rn(b.x, b.y);
     __nv_bfloat162 p3 = __floats2bfloat162_rn(b.z, b.w);
-    uint4 v;
-    v.x = *reinterpret_cast<uint32_t*>(&p0);
-    v.y = *reinterpret_cast<uint32_t*>(&p1);
-    v.z = *reinterpret_cast<uint32_t*>(&p2);
-    v.w = *reinterpret_cast<uint32_t*>(&p3);
-    *reinterpret_cast<uint4*>(dst + t * d_st + int64_t(h) * d_sh + c * 8) = v;
-}
-
-// src fp32 [L, H, D] contiguous -> dst bf16 [L, H, D] strided, dst = bf16_rne(src * scale)
-template <int D>
-__global__ void __launch_bounds__(256)
-acc_to_bf16_kernel(const float* __restrict__ src, __nv_bfloat16* __restrict__ dst, int64_t d_st,
-                   int64_t d_sh, int64_t L, int H, float scale) {
-    constexpr int TPR = D / 8;
-    const int64_t gid = int64_t(blockIdx.x) * 256 + threadIdx.x;
-    const int64_t row = gid / TPR;  // t * H + h
-    const int c = int(gid % TPR);
-    if (row >= L * H) return;
-    const int64_t t = row / H;
-    const int h = int(row % H);
-    const float4 a = *reinterpret_cast<const float4*>(src + row * D + c * 8);
-    const float4 b = *reinterpret_cast<const float4*>(src + row * D + c * 8 + 4);
-    __nv_bfloat162 p0 = __floats2bfloat162_rn(a.x * scale, a.y * scale);
-    __nv_bfloat162 p1 = __floats2bfloat162_rn(a.z * scale, a.w * scale);
-    __nv_bfloat162 p2 = __floats2bfloat162_rn(b.x * scale, b.y * scale);
-    __nv_bfloat162 p3 = __floats2bfloat162_rn(b.z * scale, b.w * scale);
     uint4 v;
     v.x = *reinterpret_cast<uint32_t*>(&p0);
     v.y = *reinterpret_cast<uint32_t*>(&p1);

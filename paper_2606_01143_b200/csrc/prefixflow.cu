@@ -23,6 +23,7 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t,
                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 constexpr int64_t kAlign = 256;
+constexpr size_t kMaxProfRecords = 1 << 16;   // unread profiling records kept per context
 inline int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
 
 }  // namespace
@@ -46,6 +47,11 @@ struct pf_ctx {
     char err[512] = {0};
 };
 
+// K and V tensor maps of one KV source with one box height
+struct KvMaps {
+    CUtensorMap k, v;
+};
+
 struct pf_group {
     pf_ctx* ctx;
     pf_desc desc;
@@ -59,6 +65,9 @@ struct pf_group {
     int64_t ws_cap;  // padded token positions the workspace holds (multiple of 64)
     pf::PrefixRanges pre;  // visible ranges of the prefix source (default: [0, Lp))
     int state;  // 0 begun, 1 A done, 2 C done
+    // descriptor cache: the tensor maps of the borrowed cache tensors are encoded once per group
+    KvMaps kv64, kv128;    // K1/V1 with 64-row boxes (forward) and 128-row boxes (backward)
+    KvMaps acc;            // gK1 / gV1 reduce-add maps (valid when gK1 != NULL)
 };
 
 namespace {
@@ -98,17 +107,34 @@ struct ProfScope {
     ProfRec r{nullptr, nullptr, 0};
     ProfScope(pf_ctx* c, int kind, cudaStream_t st) : ctx(c), s(st) {
         if (!ctx->profile) return;
+        if (ctx->prof.size() >= kMaxProfRecords) return;   // nobody is reading: stop recording
         r.kind = kind;
         r.a = prof_event(ctx);
         r.b = prof_event(ctx);
-        if (r.a) cudaEventRecord(r.a, s);
+        if (!r.a || !r.b) {                                // keep the one that was created
+            if (r.a) ctx->ev_pool.push_back(r.a);
+            if (r.b) ctx->ev_pool.push_back(r.b);
+            r.a = r.b = nullptr;
+            return;
+        }
+        cudaEventRecord(r.a, s);
     }
     ~ProfScope() {
-        if (!ctx->profile || !r.a || !r.b) return;
+        if (!r.a || !r.b) return;
         cudaEventRecord(r.b, s);
         ctx->prof.push_back(r);
     }
 };
+
+// The context is bound to one device: launches, memsets and tensor-map encodes must run with that
+// device current (the header's contract); a mismatch is the caller's phase/order error.
+pf_status check_device(pf_ctx* ctx) {
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess) return fail(ctx, PF_CUDA_ERROR, "cudaGetDevice failed");
+    if (cur != ctx->device)
+        return fail(ctx, PF_STATE, "current CUDA device %d is not the context's device %d", cur, ctx->device);
+    return PF_OK;
+}
 
 pf_status check_desc(pf_ctx* ctx, const pf_desc* d) {
     if (!d) return fail(ctx, PF_INVALID_ARG, "desc is NULL");
@@ -234,6 +260,7 @@ pf::PrefixRanges whole_prefix(int64_t Lp) {
         r.n = 1;
         r.len[0] = int(Lp);
         r.tile0[1] = int((Lp + 127) / 128);
+        r.sub0[1] = int((Lp + 63) / 64);
     }
     return r;
 }
@@ -254,25 +281,25 @@ pf::SeqTable make_seq_table(int n, const int64_t* cu) {
 
 // ---- forward launch over n sequences packed along the token axis: the queries of sequence s
 // attend to the prefix source [Lp] (all visible) + the keys of s causally
+// `prefix`: cached maps of the prefix source (NULL when Lp = 0); `causal`: cached maps of the causal
+// source when it is the group's own K1/V1 (Phase A), else NULL and K2/V2 are encoded here.
 template <int D>
-pf_status launch_fwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const pf_tensor& V1,
-                     int64_t Lp, const pf_tensor& K2, const pf_tensor& V2, const pf_tensor& O,
+pf_status launch_fwd(pf_group* g, const pf_tensor& Q, const KvMaps* prefix, int64_t Lp,
+                     const KvMaps* causal, const pf_tensor& K2, const pf_tensor& V2, const pf_tensor& O,
                      float* LSE, int64_t lse_stride, int n, const int64_t* cu, int prof_kind,
                      cudaStream_t s) {
     pf_ctx* ctx = g->ctx;
     const int Hq = g->desc.n_q_heads, Hkv = g->desc.n_kv_heads;
     const int64_t total = cu[n];
-    CUtensorMap mK1, mV1, mK2, mV2;
+    KvMaps own;
     pf_status st;
-    if ((st = make_map(ctx, &mK2, "K", K2, total, Hkv, D))) return st;
-    if ((st = make_map(ctx, &mV2, "V", V2, total, Hkv, D))) return st;
-    if (Lp > 0) {
-        if ((st = make_map(ctx, &mK1, "K1", K1, Lp, Hkv, D))) return st;
-        if ((st = make_map(ctx, &mV1, "V1", V1, Lp, Hkv, D))) return st;
-    } else {
-        mK1 = mK2;
-        mV1 = mV2;
+    if (!causal) {
+        if ((st = make_map(ctx, &own.k, "K", K2, total, Hkv, D, 64))) return st;
+        if ((st = make_map(ctx, &own.v, "V", V2, total, Hkv, D, 64))) return st;
+        causal = &own;
     }
+    if (Lp == 0 || !prefix) prefix = causal;
+    const CUtensorMap &mK1 = prefix->k, &mV1 = prefix->v, &mK2 = causal->k, &mV2 = causal->v;
     pf::FwdParams p;
     p.Q = static_cast<const __nv_bfloat16*>(Q.ptr);
     p.q_stride_tok = Q.stride_tok;
@@ -288,8 +315,8 @@ pf_status launch_fwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const
     p.G = Hq / Hkv;
     p.scale_log2 = g->sigma * 1.4426950408889634f;
     p.seq = make_seq_table(n, cu);
-    int ctas = 0;
-    for (int i = 0; i < n; ++i) ctas += (p.seq.ckt[i + 1] - p.seq.ckt[i]) * p.G;
+    int ctas = 0;   // one CTA per (pair of 128-row blocks, query head of the KV head's group)
+    for (int i = 0; i < n; ++i) ctas += (p.seq.ckt[i + 1] - p.seq.ckt[i] + 1) / 2 * p.G;
     if (ctas == 0) return PF_OK;
     dim3 grid(ctas, Hkv);
     {
@@ -306,11 +333,14 @@ pf_status launch_fwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const
 // source accumulate into accK1/accV1 (fp32, +=), keys of the causal source into accK2/accV2
 // (fp32 [total, Hkv, d], +=); dQ goes through the fp32 tile workspace and is rounded to bf16 once
 // all key tiles have contributed.
+// `prefix` / `prefix_acc`: cached maps of the prefix source and of its accumulators (NULL when
+// Lp = 0); `causal` / `causal_acc`: cached maps when the causal source is the group's own K1/V1 and
+// gK1/gV1 (Phase C), else NULL and K2/V2/accK2/accV2 are encoded here.
 template <int D>
-pf_status launch_bwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const pf_tensor& V1,
-                     int64_t Lp, const pf_tensor& K2, const pf_tensor& V2, const pf_tensor& O,
-                     const float* LSE, int64_t lse_stride, const pf_tensor& dO, float* accK1,
-                     float* accV1, float* accK2, float* accV2, const pf_tensor& dQ, int n,
+pf_status launch_bwd(pf_group* g, const pf_tensor& Q, const KvMaps* prefix, const KvMaps* prefix_acc,
+                     int64_t Lp, const KvMaps* causal, const KvMaps* causal_acc, const pf_tensor& K2,
+                     const pf_tensor& V2, const pf_tensor& O, const float* LSE, int64_t lse_stride,
+                     const pf_tensor& dO, float* accK2, float* accV2, const pf_tensor& dQ, int n,
                      const int64_t* cu, int prof_kind, cudaStream_t s) {
     pf_ctx* ctx = g->ctx;
     const int Hq = g->desc.n_q_heads, Hkv = g->desc.n_kv_heads, G = Hq / Hkv;
@@ -326,22 +356,27 @@ pf_status launch_bwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const
     float* delta = reinterpret_cast<float*>(g->ws + w.off_delta);
     float* dqacc = reinterpret_cast<float*>(g->ws + w.off_dq);
 
-    CUtensorMap mQ, mdO, mK1, mV1, mK2, mV2, mAK1, mAV1, mAK2, mAV2;
+    CUtensorMap mQ, mdO;
+    KvMaps own, own_acc;
     pf_status st;
     if ((st = make_map(ctx, &mQ, "Q", Q, total, Hq, D, 64))) return st;
     if ((st = make_map(ctx, &mdO, "dO", dO, total, Hq, D, 64))) return st;
-    if ((st = make_map(ctx, &mK2, "K", K2, total, Hkv, D))) return st;
-    if ((st = make_map(ctx, &mV2, "V", V2, total, Hkv, D))) return st;
-    if ((st = make_acc_map(ctx, &mAK2, "accK2", accK2, total, Hkv, D))) return st;
-    if ((st = make_acc_map(ctx, &mAV2, "accV2", accV2, total, Hkv, D))) return st;
-    if (Lp > 0) {
-        if ((st = make_map(ctx, &mK1, "K1", K1, Lp, Hkv, D))) return st;
-        if ((st = make_map(ctx, &mV1, "V1", V1, Lp, Hkv, D))) return st;
-        if ((st = make_acc_map(ctx, &mAK1, "gK1", accK1, Lp, Hkv, D))) return st;
-        if ((st = make_acc_map(ctx, &mAV1, "gV1", accV1, Lp, Hkv, D))) return st;
-    } else {
-        mK1 = mK2; mV1 = mV2; mAK1 = mAK2; mAV1 = mAV2;
+    if (!causal) {
+        if ((st = make_map(ctx, &own.k, "K", K2, total, Hkv, D))) return st;
+        if ((st = make_map(ctx, &own.v, "V", V2, total, Hkv, D))) return st;
+        causal = &own;
     }
+    if (!causal_acc) {
+        if ((st = make_acc_map(ctx, &own_acc.k, "accK2", accK2, total, Hkv, D))) return st;
+        if ((st = make_acc_map(ctx, &own_acc.v, "accV2", accV2, total, Hkv, D))) return st;
+        causal_acc = &own_acc;
+    }
+    if (Lp == 0 || !prefix) {
+        prefix = causal;
+        prefix_acc = causal_acc;
+    }
+    const CUtensorMap &mK1 = prefix->k, &mV1 = prefix->v, &mK2 = causal->k, &mV2 = causal->v;
+    const CUtensorMap &mAK1 = prefix_acc->k, &mAV1 = prefix_acc->v, &mAK2 = causal_acc->k, &mAV2 = causal_acc->v;
     PF_CUDA(ctx, cudaMemsetAsync(dqacc, 0, size_t(npad) * Hq * D * 4, s));
     {
         const int64_t threads = npad * (D / 8);
@@ -389,12 +424,14 @@ pf_status launch_bwd(pf_group* g, const pf_tensor& Q, const pf_tensor& K1, const
     p.sigma = g->sigma;
     const int64_t items = int64_t(p.nItemsP) + int64_t(seq.ckt[n]) * Hkv * p.chunksC;
     if (items > 0) {
-        ProfScope prof(ctx, prof_kind, s);
-        pf::attn_bwd_kernel<D><<<unsigned(items), pf::BwdCfg<D>::THREADS, pf::BwdCfg<D>::SMEM, s>>>(
-            mQ, mdO, mK1, mV1, mK2, mV2, mAK1, mAV1, mAK2, mAV2, p);
+        {
+            ProfScope prof(ctx, prof_kind, s);
+            pf::attn_bwd_kernel<D><<<unsigned(items), pf::BwdCfg<D>::THREADS, pf::BwdCfg<D>::SMEM, s>>>(
+                mQ, mdO, mK1, mV1, mK2, mV2, mAK1, mAV1, mAK2, mAV2, p);
+        }
+        PF_CUDA(ctx, cudaGetLastError());
+        ctx->n_launches += 1;
     }
-    PF_CUDA(ctx, cudaGetLastError());
-    ctx->n_launches += 1;
     if (nQS > 0) {
         pf::dq_finish_kernel<D><<<dim3(nQS, Hq), 256, 0, s>>>(
             dqacc, static_cast<__nv_bfloat16*>(dQ.ptr), dQ.stride_tok, dQ.stride_head, g->sigma, seq);
@@ -449,13 +486,18 @@ pf_status pf_create(pf_ctx** out, int32_t device) {
     pf_ctx* ctx = new (std::nothrow) pf_ctx();
     if (!ctx) return PF_CUDA_ERROR;
     ctx->device = device;
-    cudaError_t e = cudaSetDevice(device);
+    int prev = -1;
+    cudaError_t e = cudaGetDevice(&prev);
+    if (e == cudaSuccess) e = cudaSetDevice(device);
     cudaDeviceProp prop;
     if (e == cudaSuccess) e = cudaGetDeviceProperties(&prop, device);
     if (e != cudaSuccess) {
+        if (prev >= 0) cudaSetDevice(prev);
         delete ctx;
         return PF_CUDA_ERROR;
     }
+    // the caller's current device is restored on every exit path below
+    struct Restore { int d; ~Restore() { if (d >= 0) cudaSetDevice(d); } } restore{prev};
     if (prop.major != 10) {  // the kernels are sm_100a only: no fallback path exists
         delete ctx;
         return PF_UNSUPPORTED;
@@ -511,6 +553,11 @@ pf_status pf_set_option(pf_ctx* ctx, const char* name, int64_t value) {
 int64_t pf_counter(const pf_ctx* ctx, const char* name) {
     if (!ctx || !name) return -1;
     if (strcmp(name, "kernel_launches") == 0) return ctx->n_launches;
+    if (strcmp(name, "fwd_rescale_rows") == 0) {   // device-side debug counter (synchronises)
+        unsigned long long v = 0;
+        if (cudaMemcpyFromSymbol(&v, pf::g_fwd_rescale_rows, sizeof(v)) != cudaSuccess) return -1;
+        return int64_t(v);
+    }
     return -1;
 }
 
@@ -519,17 +566,21 @@ pf_status pf_profile_read(pf_ctx* ctx, int32_t kind, int64_t* launches, double* 
     if (!launches || !total_ms) return fail(ctx, PF_INVALID_ARG, "pf_profile_read: NULL output");
     int64_t n = 0;
     double ms = 0.0;
+    // first pass reads (no state is changed if a CUDA call fails), second pass recycles
+    for (auto& r : ctx->prof) {
+        if (r.kind != kind) continue;
+        PF_CUDA(ctx, cudaEventSynchronize(r.b));
+        float t = 0.f;
+        PF_CUDA(ctx, cudaEventElapsedTime(&t, r.a, r.b));
+        ms += t;
+        n += 1;
+    }
     std::vector<ProfRec> keep;
     for (auto& r : ctx->prof) {
         if (r.kind != kind) {
             keep.push_back(r);
             continue;
         }
-        PF_CUDA(ctx, cudaEventSynchronize(r.b));
-        float t = 0.f;
-        PF_CUDA(ctx, cudaEventElapsedTime(&t, r.a, r.b));
-        ms += t;
-        n += 1;
         ctx->ev_pool.push_back(r.a);
         ctx->ev_pool.push_back(r.b);
     }
@@ -556,6 +607,7 @@ pf_status pf_group_begin(pf_ctx* ctx, const pf_desc* desc, int64_t Lp, pf_tensor
     if (!out) return fail(ctx, PF_INVALID_ARG, "out is NULL");
     *out = nullptr;
     pf_status st;
+    if ((st = check_device(ctx))) return st;
     if ((st = check_desc(ctx, desc))) return st;
     if (Lp < 0 || Lp > (int64_t(1) << 30)) return fail(ctx, PF_INVALID_ARG, "Lp=%lld out of range", (long long)Lp);
     const int Hkv = desc->n_kv_heads, d = desc->head_dim;
@@ -594,6 +646,15 @@ pf_status pf_group_begin(pf_ctx* ctx, const pf_desc* desc, int64_t Lp, pf_tensor
     g->ws_cap = ws_capacity(*desc, workspace_bytes);
     g->pre = whole_prefix(Lp);
     g->state = 0;
+    if (Lp > 0) {
+        pf_status ms;
+        if ((ms = make_map(ctx, &g->kv64.k, "K1", K1, Lp, Hkv, d, 64)) || (ms = make_map(ctx, &g->kv64.v, "V1", V1, Lp, Hkv, d, 64)) ||
+            (ms = make_map(ctx, &g->kv128.k, "K1", K1, Lp, Hkv, d, 128)) || (ms = make_map(ctx, &g->kv128.v, "V1", V1, Lp, Hkv, d, 128)) ||
+            (ms = make_acc_map(ctx, &g->acc.k, "gK1", g->gK1, Lp, Hkv, d)) || (ms = make_acc_map(ctx, &g->acc.v, "gV1", g->gV1, Lp, Hkv, d))) {
+            delete g;
+            return ms;
+        }
+    }
     if (g->gK1 && Lp > 0 && ctx->zero_accumulators) {
         cudaStream_t s = static_cast<cudaStream_t>(stream);
         const size_t bytes = size_t(Lp) * Hkv * d * 4;
@@ -621,29 +682,29 @@ pf_status pf_phaseA_fwd(pf_group* grp, pf_tensor Q1, pf_tensor O1, float* LSE1, 
     const int Hq = grp->desc.n_q_heads, d = grp->desc.head_dim;
     const int64_t Lp = grp->Lp;
     pf_status st;
+    if ((st = check_device(ctx))) return st;
     if ((st = check_tensor(ctx, "Q1", Q1, Lp, Hq, d))) return st;
     if ((st = check_tensor(ctx, "O1", O1, Lp, Hq, d))) return st;
     if (Lp > 0 && !LSE1) return fail(ctx, PF_INVALID_ARG, "LSE1 is NULL");
     if (Lp > 0) {
         cudaStream_t s = static_cast<cudaStream_t>(stream);
-        pf_tensor none = {nullptr, 0, 0};
         const int64_t cu[2] = {0, Lp};
-        st = d == 64 ? launch_fwd<64>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, 1, cu, 0, s)
-                     : launch_fwd<128>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, 1, cu, 0, s);
+        st = d == 64 ? launch_fwd<64>(grp, Q1, nullptr, 0, &grp->kv64, grp->K1, grp->V1, O1, LSE1, Lp, 1, cu, 0, s)
+                     : launch_fwd<128>(grp, Q1, nullptr, 0, &grp->kv64, grp->K1, grp->V1, O1, LSE1, Lp, 1, cu, 0, s);
         if (st) return st;
     }
     grp->state = 1;
     return PF_OK;
 }
 
-pf_status pf_phaseB_fwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens_dev,
-                        const int32_t* cu_seqlens_host, pf_tensor Q2, pf_tensor K2, pf_tensor V2,
-                        pf_tensor O2, float* LSE2, void* stream) {
-    (void)cu_seqlens_dev;
+pf_status pf_phaseB_fwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens_host,
+                        pf_tensor Q2, pf_tensor K2, pf_tensor V2, pf_tensor O2, float* LSE2,
+                        void* stream) {
     if (!grp) return PF_INVALID_ARG;
     pf_ctx* ctx = grp->ctx;
     if (grp->state != 1) return fail(ctx, PF_STATE, "pf_phaseB_fwd needs Phase A done and Phase C not yet run");
     pf_status st;
+    if ((st = check_device(ctx))) return st;
     if ((st = check_cu(ctx, n_seqs, cu_seqlens_host))) return st;
     const int Hq = grp->desc.n_q_heads, Hkv = grp->desc.n_kv_heads, d = grp->desc.head_dim;
     const int64_t total = cu_seqlens_host[n_seqs];
@@ -667,24 +728,23 @@ pf_status pf_phaseB_fwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens
         if (n == 0) break;
         const pf_tensor q = tok_offset(Q2, t0), k = tok_offset(K2, t0), v = tok_offset(V2, t0),
                         o = tok_offset(O2, t0);
-        st = d == 64 ? launch_fwd<64>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, n, cu, 1, s)
-                     : launch_fwd<128>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, n, cu, 1, s);
+        st = d == 64 ? launch_fwd<64>(grp, q, &grp->kv64, grp->Lp, nullptr, k, v, o, LSE2 + t0, total, n, cu, 1, s)
+                     : launch_fwd<128>(grp, q, &grp->kv64, grp->Lp, nullptr, k, v, o, LSE2 + t0, total, n, cu, 1, s);
         if (st) return st;
     }
     return PF_OK;
 }
 
-pf_status pf_phaseB_bwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens_dev,
-                        const int32_t* cu_seqlens_host, pf_tensor Q2, pf_tensor K2, pf_tensor V2,
-                        pf_tensor O2, const float* LSE2, pf_tensor dO2, pf_tensor dQ2,
-                        pf_tensor dK2, pf_tensor dV2, void* stream) {
-    (void)cu_seqlens_dev;
+pf_status pf_phaseB_bwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens_host,
+                        pf_tensor Q2, pf_tensor K2, pf_tensor V2, pf_tensor O2, const float* LSE2,
+                        pf_tensor dO2, pf_tensor dQ2, pf_tensor dK2, pf_tensor dV2, void* stream) {
     if (!grp) return PF_INVALID_ARG;
     pf_ctx* ctx = grp->ctx;
     if (grp->state != 1) return fail(ctx, PF_STATE, "pf_phaseB_bwd needs Phase A done and Phase C not yet run");
     if (!grp->gK1 && grp->Lp > 0)
         return fail(ctx, PF_STATE, "pf_phaseB_bwd: the group was opened without gK1/gV1");
     pf_status st;
+    if ((st = check_device(ctx))) return st;
     if ((st = check_cu(ctx, n_seqs, cu_seqlens_host))) return st;
     const int Hq = grp->desc.n_q_heads, Hkv = grp->desc.n_kv_heads, d = grp->desc.head_dim;
     const int64_t total = cu_seqlens_host[n_seqs];
@@ -697,6 +757,15 @@ pf_status pf_phaseB_bwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens
     if ((st = check_tensor(ctx, "dK2", dK2, total, Hkv, d))) return st;
     if ((st = check_tensor(ctx, "dV2", dV2, total, Hkv, d))) return st;
     if (total > 0 && !LSE2) return fail(ctx, PF_INVALID_ARG, "LSE2 is NULL");
+    // every suffix must fit the workspace on its own (a wave is cut between suffixes, never inside
+    // one): checked for the whole call BEFORE anything is enqueued, so that a PF_WORKSPACE return
+    // leaves gK1/gV1 and the outputs untouched
+    for (int i = 0; i < n_seqs; ++i) {
+        const int64_t Ls = int64_t(cu_seqlens_host[i + 1]) - cu_seqlens_host[i];
+        if (align_up(Ls, 64) > grp->ws_cap)
+            return fail(ctx, PF_WORKSPACE, "workspace too small for suffix %d of %lld tokens (capacity %lld padded positions)",
+                        i, (long long)Ls, (long long)grp->ws_cap);
+    }
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const WsLayout w = ws_layout(grp->desc, grp->ws_cap);
     float* ak = reinterpret_cast<float*>(grp->ws + w.off_ak);
@@ -726,12 +795,12 @@ pf_status pf_phaseB_bwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens
         const pf_tensor q = tok_offset(Q2, t0), k = tok_offset(K2, t0), v = tok_offset(V2, t0),
                         o = tok_offset(O2, t0), dout = tok_offset(dO2, t0), dq = tok_offset(dQ2, t0);
         if (d == 64) {
-            st = launch_bwd<64>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, dout,
-                                grp->gK1, grp->gV1, ak, av, dq, n, cu, 2, s);
+            st = launch_bwd<64>(grp, q, &grp->kv128, &grp->acc, grp->Lp, nullptr, nullptr, k, v, o,
+                                LSE2 + t0, total, dout, ak, av, dq, n, cu, 2, s);
             if (!st) st = launch_convert_kv2<64>(grp, ak, tok_offset(dK2, t0), av, tok_offset(dV2, t0), tot, s);
         } else {
-            st = launch_bwd<128>(grp, q, grp->K1, grp->V1, grp->Lp, k, v, o, LSE2 + t0, total, dout,
-                                 grp->gK1, grp->gV1, ak, av, dq, n, cu, 2, s);
+            st = launch_bwd<128>(grp, q, &grp->kv128, &grp->acc, grp->Lp, nullptr, nullptr, k, v, o,
+                                 LSE2 + t0, total, dout, ak, av, dq, n, cu, 2, s);
             if (!st) st = launch_convert_kv2<128>(grp, ak, tok_offset(dK2, t0), av, tok_offset(dV2, t0), tot, s);
         }
         if (st) return st;
@@ -757,6 +826,7 @@ pf_status pf_group_set_prefix_ranges(pf_group* grp, int32_t n_ranges, const int6
         r.start[r.n] = int(starts_host[i]);
         r.len[r.n] = int(lens_host[i]);
         r.tile0[r.n + 1] = r.tile0[r.n] + int((lens_host[i] + 127) / 128);
+        r.sub0[r.n + 1] = r.sub0[r.n] + int((lens_host[i] + 63) / 64);
         end = starts_host[i] + lens_host[i];
         ++r.n;
     }
@@ -782,6 +852,7 @@ pf_status pf_segment_bwd(pf_group* grp, int64_t Ls, pf_tensor Q, pf_tensor K, pf
     if (Ls == 0) return PF_OK;
     const int Hq = grp->desc.n_q_heads, Hkv = grp->desc.n_kv_heads, d = grp->desc.head_dim;
     pf_status st;
+    if ((st = check_device(ctx))) return st;
     if ((st = check_tensor(ctx, "Q", Q, Ls, Hq, d))) return st;
     if ((st = check_tensor(ctx, "K", K, Ls, Hkv, d))) return st;
     if ((st = check_tensor(ctx, "V", V, Ls, Hkv, d))) return st;
@@ -798,12 +869,12 @@ pf_status pf_segment_bwd(pf_group* grp, int64_t Ls, pf_tensor Q, pf_tensor K, pf
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     const int64_t cu[2] = {0, Ls};
     if (d == 64) {
-        st = launch_bwd<64>(grp, Q, grp->K1, grp->V1, grp->Lp, K, V, O, LSE, Ls, dO, grp->gK1, grp->gV1,
-                            accK, accV, dQ, 1, cu, 2, s);
+        st = launch_bwd<64>(grp, Q, &grp->kv128, &grp->acc, grp->Lp, nullptr, nullptr, K, V, O, LSE, Ls,
+                            dO, accK, accV, dQ, 1, cu, 2, s);
         if (!st) st = launch_convert_kv2<64>(grp, accK, dK, accV, dV, Ls, s);
     } else {
-        st = launch_bwd<128>(grp, Q, grp->K1, grp->V1, grp->Lp, K, V, O, LSE, Ls, dO, grp->gK1, grp->gV1,
-                             accK, accV, dQ, 1, cu, 2, s);
+        st = launch_bwd<128>(grp, Q, &grp->kv128, &grp->acc, grp->Lp, nullptr, nullptr, K, V, O, LSE, Ls,
+                             dO, accK, accV, dQ, 1, cu, 2, s);
         if (!st) st = launch_convert_kv2<128>(grp, accK, dK, accV, dV, Ls, s);
     }
     return st;
@@ -817,6 +888,7 @@ pf_status pf_phaseC_bwd(pf_group* grp, pf_tensor Q1, pf_tensor O1, const float* 
     const int Hq = grp->desc.n_q_heads, Hkv = grp->desc.n_kv_heads, d = grp->desc.head_dim;
     const int64_t Lp = grp->Lp;
     pf_status st;
+    if ((st = check_device(ctx))) return st;
     if ((st = check_tensor(ctx, "Q1", Q1, Lp, Hq, d))) return st;
     if ((st = check_tensor(ctx, "O1", O1, Lp, Hq, d))) return st;
     if ((st = check_tensor(ctx, "dO1", dO1, Lp, Hq, d))) return st;
@@ -837,15 +909,15 @@ pf_status pf_phaseC_bwd(pf_group* grp, pf_tensor Q1, pf_tensor O1, const float* 
             PF_CUDA(ctx, cudaMemsetAsync(ak, 0, kvb, s));
             PF_CUDA(ctx, cudaMemsetAsync(av, 0, kvb, s));
         }
-        pf_tensor none = {nullptr, 0, 0};
         const int64_t cu[2] = {0, Lp};
+        const KvMaps* cacc = grp->gK1 ? &grp->acc : nullptr;   // replay: workspace accumulators, encoded per call
         if (d == 64) {
-            st = launch_bwd<64>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, dO1, nullptr,
-                                nullptr, ak, av, dQ1, 1, cu, 3, s);
+            st = launch_bwd<64>(grp, Q1, nullptr, nullptr, 0, &grp->kv128, cacc, grp->K1, grp->V1, O1, LSE1,
+                                Lp, dO1, ak, av, dQ1, 1, cu, 3, s);
             if (!st) st = launch_convert_kv2<64>(grp, ak, dK1, av, dV1, Lp, s);
         } else {
-            st = launch_bwd<128>(grp, Q1, none, none, 0, grp->K1, grp->V1, O1, LSE1, Lp, dO1, nullptr,
-                                 nullptr, ak, av, dQ1, 1, cu, 3, s);
+            st = launch_bwd<128>(grp, Q1, nullptr, nullptr, 0, &grp->kv128, cacc, grp->K1, grp->V1, O1, LSE1,
+                                 Lp, dO1, ak, av, dQ1, 1, cu, 3, s);
             if (!st) st = launch_convert_kv2<128>(grp, ak, dK1, av, dV1, Lp, s);
         }
         if (st) return st;
