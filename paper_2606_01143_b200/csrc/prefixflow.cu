@@ -315,8 +315,8 @@ pf_status launch_fwd(pf_group* g, const pf_tensor& Q, const KvMaps* prefix, int6
     p.G = Hq / Hkv;
     p.scale_log2 = g->sigma * 1.4426950408889634f;
     p.seq = make_seq_table(n, cu);
-    int ctas = 0;   // one CTA per (pair of 128-row blocks, query head of the KV head's group)
-    for (int i = 0; i < n; ++i) ctas += (p.seq.ckt[i + 1] - p.seq.ckt[i] + 1) / 2 * p.G;
+    int ctas = 0;   // one CTA per (128-row block, query head of the KV head's group)
+    for (int i = 0; i < n; ++i) ctas += (p.seq.ckt[i + 1] - p.seq.ckt[i]) * p.G;
     if (ctas == 0) return PF_OK;
     dim3 grid(ctas, Hkv);
     {

@@ -44,16 +44,16 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
     uint32_t ok;
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
         "selp.u32 %0, 1, 0, p;\n\t}\n"
         : "=r"(ok)
-        : "r"(smem_u32(bar)), "r"(parity)
+        : "r"(smem_u32(bar)), "r"(parity), "r"(0x989680u)   // suspend-time hint: sleep in hardware, do not spin
         : "memory");
     return ok != 0;
 }
-// Spin on try_wait (which itself suspends for a HW-defined time).  A wait that never completes is
-// a pipeline bug: trap after ~2^26 failed polls (seconds) so that it surfaces as a CUDA error
-// instead of a hung GPU.
+// Loop on try_wait (which suspends the thread in hardware up to the time hint, so that waiting warps
+// do not take issue slots from the working ones).  A wait that never completes is a pipeline bug:
+// trap after 2^26 failed polls so that it surfaces as a CUDA error instead of a hung GPU.
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     uint32_t polls = 0;
     while (!mbar_try_wait(bar, parity)) {

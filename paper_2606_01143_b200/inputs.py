@@ -15,10 +15,10 @@ keys exceeds everything before them by ~0.75 sqrt(d) nats (> 8 in log2 units) fo
 an online softmax must re-reference its running maximum there, several tiles into the sequence.
 "ramp" adds a * u to every query row and a * (position / T) * u to key row `position` (prefix
 positions 0..Lp-1, suffix positions continue at Lp; T = Lp + longest suffix; a = sqrt(RAMP_NATS /
-sqrt(d)) ~ 2): the scaled scores of every row grow linearly by RAMP_NATS = 48 nats (69 log2 units)
-over the sequence, so the running maximum is re-referenced ~8 times per row, spread over the whole
+sqrt(d)) ~ 1.5): the scaled scores of every row grow linearly by RAMP_NATS = 24 nats (35 log2 units)
+over the sequence, so the running maximum is re-referenced ~4 times per row, spread over the whole
 KV loop, while the softmax mass stays on many recent keys and the gradients keep a healthy
-magnitude.  The planted component is kept at ~2x the noise on purpose: a key (query) component of
+magnitude.  The planted component is kept at ~1.5x the noise on purpose: a key (query) component of
 norm a multiplies the bf16 rounding of dS into dQ (dK) by a, which is rounding of the bf16
 contract, not of a kernel.
 Layout is token-major [L, H, d] with d contiguous (SURVEY.md §8c reading 7).
@@ -96,7 +96,7 @@ def _spike_direction(seed: int, Hkv: int, d: int) -> torch.Tensor:
     return (torch.randint(0, 2, (Hkv, d), generator=g).to(torch.float32) * 2.0 - 1.0)
 
 
-RAMP_NATS = 48.0
+RAMP_NATS = 24.0
 
 
 def ramp_amplitude(d: int) -> float:

@@ -114,7 +114,7 @@ def test_smallest_nonempty(ctx):
 ])
 @pytest.mark.parametrize("dist", ["ramp", "spike"])
 def test_adversarial_logits(ctx, Hq, Hkv, d, Lp, Ls, wave, dist):
-    """Inputs whose row maximum keeps growing late in the sequence (inputs.py "ramp": 69 log2 units
+    """Inputs whose row maximum keeps growing late in the sequence (inputs.py "ramp": 35 log2 units
     over the sequence for every row; "spike": planted keys late in the prefix and late in each suffix), so
     that the forward kernel must re-base its running softmax maximum and rescale the O accumulator
     many tiles into the KV loop -- the path N(0,1) logits never reach.  The debug counter proves
@@ -127,7 +127,7 @@ def test_adversarial_logits(ctx, Hq, Hkv, d, Lp, Ls, wave, dist):
                     backward=(dist == "ramp"))
     n1 = pf.pf_counter(ctx, "fwd_rescale_rows")
     rows = (Lp + sum(Ls)) * Hq
-    assert n1 - n0 >= (rows * 2 if dist == "ramp" else rows // 2), (n0, n1, rows)
+    assert n1 - n0 >= (rows if dist == "ramp" else rows // 2), (n0, n1, rows)
 
 
 @pytest.mark.parametrize("items", [(1, 1), (2, 3), (7, 7), (1000, 1000)])
