@@ -230,6 +230,131 @@ def workload_config(shape, name: str) -> dict:
 
 
 # --------------------------------------------------------------------------------------------------
+# helper legs of the GPU arm
+# --------------------------------------------------------------------------------------------------
+def _strip(r: dict) -> dict:
+    r = dict(r)
+    r.pop("outputs", None)
+    return r
+
+
+def memory_legs(ctx, lifecycle, shape, dev, wave: int, layers: int, reps: int = 2) -> dict:
+    """Lifecycle measurement of one layer and of an L-layer pipeline: dormant sets resident
+    ("none"), offloaded with Phase B waiting for the copy ("wait": every wave runs with the set out
+    of HBM) and offloaded without any wait ("overlap").  Inputs are drawn on the device as the
+    schedule asks for them (lifecycle.RandomSource): the times hold no host upload."""
+    import torch
+    out = dict(wave=wave, dormant_bytes_per_layer=lifecycle.dormant_bytes(shape),
+               note="tensors allocated and freed as a trainer would (suffix-wave tensors live only during their "
+                    "wave); peaks are torch.cuda.max_memory_allocated; pinned pool = 1.5x the dormant footprint")
+    for L in ([1] + ([layers] if layers > 1 else [])):
+        pool = lifecycle.PinnedPool(int(1.5 * L * lifecycle.dormant_bytes(shape)))
+        side = torch.cuda.Stream(dev)
+        res = {}
+        for mode in ("none", "wait", "overlap"):
+            for _ in range(reps):
+                r = lifecycle.run_layers(ctx, lifecycle.RandomSource(shape, L, dev, seed=7), dev, wave=wave,
+                                         offload=mode, pool=pool, side=side, early_prefetch=(mode == "overlap"))
+            res[mode] = _strip(r)
+            torch.cuda.empty_cache()
+        leg = dict(layers=L, resident=res["none"], offload_wait=res["wait"], offload_overlap=res["overlap"],
+                   phaseB_peak_reduction_pct=100.0 * (1 - res["wait"]["peak_phaseB_bytes"] / res["none"]["peak_phaseB_bytes"]),
+                   ms_ratio_wait=res["wait"]["ms"] / res["none"]["ms"],
+                   ms_ratio_overlap=res["overlap"]["ms"] / res["none"]["ms"])
+        out["single_layer" if L == 1 else "multilayer"] = leg
+        del pool
+    return out
+
+
+def sweep_legs(ctx, schedule, lifecycle, inputs, dev, stream, peaks, steps: int = 3) -> dict:
+    """Step time vs the packed replay at the corners of configs[3] and at configs[2] / configs[4]
+    (inputs drawn on the device: timing only), plus the single-layer memory leg of configs[4]."""
+    import torch
+    out = {}
+    legs = [(f"sweep-r{r}-n{n}", inputs.config_sweep(r, n)) for r in (20, 95) for n in (2, 16)]
+    legs += [("ragged", inputs.config_ragged()), ("32k", inputs.config_32k())]
+    for name, shape in legs:
+        F = flops(shape)
+        g = schedule.random_device_group(shape, dev, wave=max(1, shape.N), seed=shape.seed)
+        step = lambda: schedule.run_prefixflow_step(ctx, g, stream)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+        def t(fn, k):
+            fn()
+            torch.cuda.synchronize()
+            e0.record(stream)
+            for _ in range(k):
+                fn()
+            e1.record(stream)
+            torch.cuda.synchronize()
+            return e0.elapsed_time(e1) / k
+        ms = t(step, steps)
+        rp = schedule.make_replay_packed(g)
+        ms_r = t(lambda: schedule.run_replay_packed_step(ctx, rp, stream), max(1, steps - 1))
+        out[name] = dict(step_ms=ms, step_tflops=F["step"] / (ms * 1e-3) / 1e12, replay_packed_ms=ms_r,
+                         speedup=ms_r / ms, ideal_speedup_pair_model=F["ideal_speedup"])
+        del g, rp
+        torch.cuda.empty_cache()
+    m = memory_legs(ctx, lifecycle, inputs.config_32k(), dev, 1, 0, reps=1)
+    out["32k"]["memory_single_layer"] = m["single_layer"]
+    return out
+
+
+def run_sharded_group(args, shape, ctx, pf, pfd, inputs, schedule, dist, dev, rank, world, peaks) -> None:
+    """N > 1, ONE rollout group over all ranks (strong scaling): --shard heads (KV-head sharding, no
+    communication) or --shard split (suffix sharding with an all-gather of K1/V1
+    and a reduce-scatter of gK1/gV1).  Prints the contract's JSON line."""
+    import torch
+    F = flops(shape)
+    inp = inputs.make_group(shape)
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        torch.cuda.synchronize()
+        dist.barrier()
+        torch.cuda.synchronize()
+
+    if args.shard == "heads":
+        g = schedule.to_device(inp, dev, wave=max(1, shape.N))
+        sh = schedule.head_shard(g, world, rank)
+        step = lambda: schedule.run_prefixflow_step(ctx, sh, stream)
+        extra = dict(parallelism=f"1 group over {world} ranks, KV-head sharded, no communication")
+    else:
+        plan = pfd.split_plan(shape, world, rank)
+        rk = pfd.SplitGroupRank(ctx, inp, plan, dev, wave=0, stream=stream)
+        comm = pfd.DistComm()
+        cs = torch.cuda.Stream(dev)
+        waits = []
+        step = lambda: waits.append(pfd.run_split_group_step(rk, comm, cs))
+        extra = dict(parallelism=f"1 group over {world} ranks: Phase A/C head-sharded, Phase B suffix-sharded, "
+                                 f"all-gather K1/V1 + reduce-scatter gK1/gV1")
+    for _ in range(args.warmup):
+        step()
+    if args.shard == "split":
+        waits.clear()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    barrier()
+    ms = pfd.max_over_ranks(e0.elapsed_time(e1), dev) / args.steps
+    comm_ms = None
+    if args.shard == "split":
+        comm_ms = sum(a.elapsed_time(b) for w in waits for a, b in w.values()) / args.steps
+        comm_ms = pfd.max_over_ranks(comm_ms, dev)
+    cfg = workload_config(shape, args.config)
+    cfg.update(extra)
+    out = dict(metric=METRIC, value=F["step"] / (ms * 1e-3) / 1e12, unit=UNIT, n_gpus=world, steps=args.steps,
+               warmup=args.warmup, ms_per_step=ms, higher_is_better=True, scaling="strong", vs_baseline=None,
+               dtype="bf16", data="synthetic", config=cfg, shard=args.shard, exposed_comm_ms=comm_ms,
+               flops=dict(step=F["step"]), peaks=peaks)
+    if rank == 0:
+        print(json.dumps(out))
+
+
+# --------------------------------------------------------------------------------------------------
 # GPU leg
 # --------------------------------------------------------------------------------------------------
 def main() -> None:
@@ -250,6 +375,13 @@ def main() -> None:
     ap.add_argument("--no-offload", action="store_true", help="skip the memory-lifecycle / offload measurement")
     ap.add_argument("--offload-wave", type=int, default=1, help="suffixes per wave in the lifecycle measurement")
     ap.add_argument("--layers", type=int, default=4, help="attention layers in the multi-layer offload pipeline (0 = skip)")
+    ap.add_argument("--bwd-pairs", type=int, default=0, help="C-ABI option bwd_pairs_per_item (0 = heuristic)")
+    ap.add_argument("--deterministic", action="store_true", help="C-ABI option deterministic_gkv")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the compact prefix-ratio x N sweep / configs[2], configs[4] legs")
+    ap.add_argument("--shard", default="groups", choices=["groups", "heads", "split"],
+                    help="N > 1: 'groups' = one independent group per rank (weak scaling, default); 'heads' = ONE group "
+                         "sharded by KV head, no communication; 'split' = ONE group, Phase B sharded by suffix with an "
+                         "all-gather of K1/V1 and a reduce-scatter of gK1/gV1 (strong scaling)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -264,7 +396,7 @@ def main() -> None:
     import torch.distributed as dist
     from paper_2606_01143_b200 import binding as pf          # raises if libprefixflow.so is missing
     from paper_2606_01143_b200 import dist as pfd
-    from paper_2606_01143_b200 import inputs, schedule
+    from paper_2606_01143_b200 import inputs, lifecycle, schedule
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback of the product path)")
@@ -275,11 +407,20 @@ def main() -> None:
         dist.init_process_group("nccl", device_id=dev)
 
     shape = pick_config(args.config)
+    peaks = measured_peaks()
+    ctx = pf.pf_create(local_rank)
+    if args.bwd_pairs:
+        pf.pf_set_option(ctx, "bwd_pairs_per_item", args.bwd_pairs)
+    if args.deterministic:
+        pf.pf_set_option(ctx, "deterministic_gkv", 1)
+    if world > 1 and args.shard != "groups":
+        run_sharded_group(args, shape, ctx, pf, pfd, inputs, schedule, dist, dev, rank, world, peaks)
+        pf.pf_destroy(ctx)
+        dist.destroy_process_group()
+        return
     # weak scaling over independent rollout groups: rank r draws its own group
     shape = pfd.rank_shape(shape, rank)
     F = flops(shape)
-    peaks = measured_peaks()
-    ctx = pf.pf_create(local_rank)
     inp = inputs.make_group(shape)
     wave = args.wave if args.wave > 0 else max(1, shape.N)
     g = schedule.to_device(inp, dev, wave=wave)
@@ -334,19 +475,22 @@ def main() -> None:
     phaseB_tflops = tf(F["B_fwd"] + F["B_bwd"], b_ms)
     other_ms = ms_step_prof - sum(ph_ms.values())
 
-    # roofline of the dominant kernel: attn_bwd_kernel as launched by pf_phaseB_bwd
-    nB = prof["B_bwd"]["launches"]
-    ach = tf(F["B_bwd"] * steps / nB, prof["B_bwd"]["ms_per_launch"]) if nB else None
-    kname = f"attn_bwd_kernel<{shape.head_dim}>"
-    roofline = dict(bound="tensor", kernel=kname + " (pf_phaseB_bwd)", achieved=ach,
-                    peak=peaks["sustained"], unit="TFLOP/s",
-                    frac=(ach / peaks["sustained"]) if ach else None,
-                    peak_kind="bf16 sustained, " + peaks["source"],
-                    frac_of_burst=(ach / peaks["burst"]) if ach else None, peak_burst=peaks["burst"],
+    # roofline of the dominant kernel (attn_bwd_kernel as launched by pf_phaseB_bwd) and of the
+    # forward kernel (pf_phaseB_fwd).  The timed region is K steps of a few ms at full clock: the
+    # BURST peak is the denominator (a kernel timed alone / in a short region); the fraction of the
+    # sustained peak (seconds-long GEMM loop under the power cap) is printed beside it.
+    def roofline_of(kind, call, kname, fl):
+        n = prof[kind]["launches"]
+        ach = tf(fl * steps / n, prof[kind]["ms_per_launch"]) if n else None
+        return dict(bound="tensor", kernel=f"{kname} ({call})", achieved=ach, peak=peaks["burst"], unit="TFLOP/s",
+                    frac=(ach / peaks["burst"]) if ach else None,
+                    peak_kind="bf16 burst, " + peaks["source"],
+                    frac_of_sustained=(ach / peaks["sustained"]) if ach else None, peak_sustained=peaks["sustained"],
                     frac_of_nominal=(ach / 2250.0) if ach else None,
-                    flops_per_launch=F["B_bwd"] / max(1, nB // max(1, steps)) if nB else None,
-                    ms_per_launch=prof["B_bwd"]["ms_per_launch"],
-                    traffic=ncu_traffic(kname, args.config))
+                    flops_per_launch=fl / max(1, n // max(1, steps)) if n else None,
+                    ms_per_launch=prof[kind]["ms_per_launch"], traffic=ncu_traffic(kname, args.config))
+    roofline = roofline_of("B_bwd", "pf_phaseB_bwd", f"attn_bwd_kernel<{shape.head_dim}>", F["B_bwd"])
+    roofline_fwd = roofline_of("B_fwd", "pf_phaseB_fwd", f"attn_fwd_kernel<{shape.head_dim}>", F["B_fwd"])
 
     # ---- N-times replay baseline: the same kernels on every concatenated [P || S(i)] ----
     replay = None
@@ -357,10 +501,22 @@ def main() -> None:
         for _ in range(2):
             rstep()
         ms_replay = timed(rstep, rsteps)
-        replay = dict(ms_per_step=ms_replay, steps=rsteps, tflops=tf(F["replay"], ms_replay),
-                      speedup=ms_replay / ms_step, ideal_speedup_pair_model=F["ideal_speedup"])
         del r
         torch.cuda.empty_cache()
+        # the same N full sequences packed into one forward and one backward launch (Lp = 0,
+        # n_seqs = N): the baseline pays one launch tail per kernel, like the step under test
+        rp = schedule.make_replay_packed(g)
+        rpstep = lambda: schedule.run_replay_packed_step(ctx, rp, stream)
+        for _ in range(2):
+            rpstep()
+        ms_packed = timed(rpstep, rsteps)
+        del rp
+        torch.cuda.empty_cache()
+        best = min(ms_replay, ms_packed)
+        replay = dict(ms_per_step=best, steps=rsteps, tflops=tf(F["replay"], best),
+                      speedup=best / ms_step, ideal_speedup_pair_model=F["ideal_speedup"],
+                      per_sequence_ms=ms_replay, packed_ms=ms_packed,
+                      note="speedup is quoted against the FASTER of the two replay organisations")
 
     # ---- the same step with one Phase-B call per suffix (the paper's "separate" organisation) ----
     wave1 = None
@@ -387,48 +543,21 @@ def main() -> None:
         torch.cuda.empty_cache()
 
     # ---- memory lifecycle: Phase-B peak HBM with the dormant Phase-A set
-    # {Q1, O1, LSE1} resident vs offloaded to pinned host memory on a side stream ----
+    # {Q1, O1, LSE1} resident vs offloaded to a pinned host pool on a side stream ----
     memory = None
     if rank == 0 and not args.no_offload:
         del g
         torch.cuda.empty_cache()
-        pinned = {}
-        res = {}
-        for mode in (False, True):
-            schedule.run_lifecycle_step(ctx, inp, dev, wave=args.offload_wave, offload=mode, pinned=pinned)
-            r = schedule.run_lifecycle_step(ctx, inp, dev, wave=args.offload_wave, offload=mode, pinned=pinned)
-            r.pop("outputs")
-            res["offload" if mode else "resident"] = r
-            torch.cuda.empty_cache()
-        a, b = res["resident"], res["offload"]
-        memory = dict(wave=args.offload_wave, resident=a, offload=b,
-                      phaseB_peak_reduction_pct=100.0 * (1 - b["peak_phaseB_bytes"] / a["peak_phaseB_bytes"]),
-                      dormant_bytes=inp.Q1.numel() * 2 * 2 + inp.Q1.shape[0] * inp.Q1.shape[1] * 4,
-                      note="one attention layer; tensors allocated and freed as a trainer would "
-                           "(suffix-wave tensors live only during their wave); peaks are "
-                           "torch.cuda.max_memory_allocated")
-        if args.layers > 0:
-            # L layers (independent seeded groups of the same shape), offload pipeline with
-            # one-layer-ahead prefetch before Phase C
-            layers = [inp] + [inputs.make_group(pfd.rank_shape(shape, 1000 + l)) for l in range(1, args.layers)]
-            ml = {}
-            for mode in (False, True):
-                schedule.run_multilayer_step(ctx, layers, dev, wave=args.offload_wave, offload=mode, pinned=pinned)
-                r = schedule.run_multilayer_step(ctx, layers, dev, wave=args.offload_wave, offload=mode, pinned=pinned)
-                r.pop("outputs")
-                ml["offload" if mode else "resident"] = r
-                torch.cuda.empty_cache()
-            memory["multilayer"] = dict(
-                layers=args.layers, resident=ml["resident"], offload=ml["offload"],
-                phaseB_peak_reduction_pct=100.0 * (1 - ml["offload"]["peak_phaseB_bytes"] / ml["resident"]["peak_phaseB_bytes"]),
-                exposed_prefetch_ms=ml["offload"]["exposed_prefetch_ms"])
-            r = schedule.run_multilayer_step(ctx, layers, dev, wave=args.offload_wave, offload=True, pinned=pinned,
-                                             early_prefetch=True)
-            memory["multilayer"]["early_prefetch"] = dict(
-                phaseB_peak_reduction_pct=100.0 * (1 - r["peak_phaseB_bytes"] / ml["resident"]["peak_phaseB_bytes"]),
-                exposed_prefetch_ms=r["exposed_prefetch_ms"], ms=r["ms"])
-            del layers
-        pinned.clear()
+        memory = memory_legs(ctx, lifecycle, shape, dev, args.offload_wave, args.layers)
+        g = schedule.to_device(inp, dev, wave=wave)
+
+    # ---- compact sweep: the four corners of the prefix-ratio x N sweep (configs[3]) and configs[2],
+    # configs[4]: step vs replay, so that one bench line shows the trend ----
+    sweep = None
+    if rank == 0 and world == 1 and not args.no_sweep and args.config == "7b":
+        del g
+        torch.cuda.empty_cache()
+        sweep = sweep_legs(ctx, schedule, lifecycle, inputs, dev, stream, peaks)
         g = schedule.to_device(inp, dev, wave=wave)
 
     # ---- end to end: pinned host inputs -> device, step, results -> pinned host, every step ----
@@ -524,6 +653,8 @@ def main() -> None:
                    g.Q2 + g.K2 + g.V2 + g.dO2 + g.O2 + g.dQ2 + g.dK2 + g.dV2)
     cfg = workload_config(shape, args.config)
     cfg["wave"] = wave
+    if args.bwd_pairs or args.deterministic:
+        cfg["bwd_split"] = "deterministic_gkv" if args.deterministic else f"bwd_pairs_per_item={args.bwd_pairs}"
     cfg["l2"] = (f"no explicit flush: one step touches {ws_bytes / 2 ** 20:.0f} MiB of inputs+outputs "
                  f"(> 126 MiB L2) before any tensor is reused" if ws_bytes > L2_BYTES else
                  f"working set {ws_bytes / 2 ** 20:.0f} MiB fits L2 (parity-size config; not a bench line)")
@@ -531,7 +662,7 @@ def main() -> None:
         metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
         ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="bf16",
         data="synthetic", config=cfg, clocks=clk.summary(), e2e=e2e, gpu_launches=launches,
-        roofline=roofline, cpu_baseline=cpu,
+        roofline=roofline, roofline_fwd=roofline_fwd, cpu_baseline=cpu, sweep=sweep,
         phases=phases, phaseB=dict(ms=b_ms, tflops=phaseB_tflops,
                                    pct_of_bf16_burst=100 * phaseB_tflops / peaks["burst"] if phaseB_tflops else None,
                                    pct_of_bf16_sustained=100 * phaseB_tflops / peaks["sustained"] if phaseB_tflops else None,

@@ -84,6 +84,14 @@ const char* pf_last_error(const pf_ctx* ctx);
  *                      (no contention); 1 = maximal parallelism, most reduce-add traffic.
  *   "bwd_heads_per_item" : the same for the tiles of a suffix's own (causal) keys: query heads of
  *                      the KV head per CTA (0 = heuristic).
+ *   "deterministic_gkv"  : 1 = every key tile (prefix and causal) is owned by ONE CTA per launch, which
+ *                      sums all its (sequence, query head) pairs in TMEM in a fixed order and adds the
+ *                      result once: gK1 / gV1 / dK / dV are then bit-reproducible from run to run (the
+ *                      launches of a group are stream-ordered).  Fewer, longer CTAs: slower when the
+ *                      launch has few key tiles.  dQ still sums its key tiles in arrival order.
+ *                      0 (default) = the heuristic split (several CTAs may add into one key tile; the
+ *                      fp32 adds happen at L2 in arrival order, "agreement within datatype
+ *                      tolerance rather than bitwise").
  *   "zero_accumulators"  : 1 (default) = pf_group_begin zeroes gK1/gV1; 0 = it leaves them as they
  *                      are (segment-by-segment training, where they already hold the contributions
  *                      of later segments). */

@@ -41,6 +41,7 @@ struct pf_ctx {
     int bwd_heads_per_item = 0;  // query heads per causal-tile CTA; 0 = heuristic
     bool profile = false;
     bool zero_accumulators = true;
+    bool deterministic_gkv = false;  // one CTA per key tile: gK1/gV1/dK/dV sums in a fixed order
     int64_t n_launches = 0;
     std::vector<ProfRec> prof;         // recorded, not yet read
     std::vector<cudaEvent_t> ev_pool;  // recycled events
@@ -406,16 +407,18 @@ pf_status launch_bwd(pf_group* g, const pf_tensor& Q, const KvMaps* prefix, cons
     const double target = std::fmin(192.0, std::fmax(24.0, double(iters) / (6.0 * ctx->num_sms)));
     const double avg_nqs = n > 0 ? double(nQS) / n : 1.0;
     const int pairs = n * G;
-    int ppcP = ctx->bwd_pairs_per_item > 0 ? ctx->bwd_pairs_per_item
-                                           : int(std::lround(target / std::fmax(1.0, avg_nqs)));
+    int ppcP = ctx->deterministic_gkv ? pairs
+               : ctx->bwd_pairs_per_item > 0 ? ctx->bwd_pairs_per_item
+                                             : int(std::lround(target / std::fmax(1.0, avg_nqs)));
     ppcP = ppcP < 1 ? 1 : (ppcP > pairs ? pairs : ppcP);
-    if (ctx->bwd_pairs_per_item == 0 && pairs > 0) {   // even chunks: no tiny last item
+    if (ctx->bwd_pairs_per_item == 0 && !ctx->deterministic_gkv && pairs > 0) {   // even chunks: no tiny last item
         const int chunks = (pairs + ppcP - 1) / ppcP;
         ppcP = (pairs + chunks - 1) / chunks;
     }
-    int ppcC = ctx->bwd_heads_per_item > 0 ? ctx->bwd_heads_per_item
-                                           : int(std::lround(target / std::fmax(1.0, avg_nqs)));
-    const int capC = ctx->bwd_heads_per_item > 0 ? G : (G + 1) / 2;   // measured: G heads per causal item is too coarse
+    int ppcC = ctx->deterministic_gkv ? G
+               : ctx->bwd_heads_per_item > 0 ? ctx->bwd_heads_per_item
+                                             : int(std::lround(target / std::fmax(1.0, avg_nqs)));
+    const int capC = (ctx->bwd_heads_per_item > 0 || ctx->deterministic_gkv) ? G : (G + 1) / 2;   // measured: G heads per causal item is too coarse
     ppcC = ppcC < 1 ? 1 : (ppcC > capC ? capC : ppcC);
     p.ppcP = ppcP; p.chunksP = (pairs + ppcP - 1) / ppcP;
     p.ppcC = ppcC; p.chunksC = (G + ppcC - 1) / ppcC;
@@ -541,6 +544,10 @@ pf_status pf_set_option(pf_ctx* ctx, const char* name, int64_t value) {
     }
     if (strcmp(name, "zero_accumulators") == 0) {
         ctx->zero_accumulators = value != 0;
+        return PF_OK;
+    }
+    if (strcmp(name, "deterministic_gkv") == 0) {
+        ctx->deterministic_gkv = value != 0;
         return PF_OK;
     }
     if (strcmp(name, "profile") == 0) {

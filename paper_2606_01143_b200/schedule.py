@@ -3,7 +3,9 @@
 Host-side orchestration only: allocates device buffers with torch and issues the C-ABI calls of
 `binding` in the paper's order (Phase A once, Phase B fwd+bwd per suffix, Phase C once).  The
 replay baseline (BASELINE.json north_star item 3) runs the SAME kernels on each concatenated
-[P || S(i)]: a group opened with Lp = T_i and no gK1/gV1, `pf_phaseA_fwd` then `pf_phaseC_bwd`.
+[P || S(i)]: a group opened with Lp = T_i and no gK1/gV1, `pf_phaseA_fwd` then `pf_phaseC_bwd`
+(one launch pair per trajectory), or all N trajectories packed into one launch pair.  The memory
+lifecycle (offload / prefetch of the dormant Phase-A set) lives in `lifecycle.py`.
 """
 from __future__ import annotations
 
@@ -117,6 +119,51 @@ def run_prefixflow_step(ctx, g: DeviceGroup, stream=None, after_each_suffix=None
         pf.pf_group_end(grp)
 
 
+def head_shard(g: DeviceGroup, world: int, rank: int) -> DeviceGroup:
+    """KV-head shard `rank` of `world` of a device group (the paper's TP rule: each
+    rank caches its own head shard, no communication): the bf16 inputs and outputs are head slices
+    of the full group's tensors IN PLACE (strided views: the C ABI takes token / head strides), the
+    fp32 accumulators, LSE and workspace of the shard are its own.  Running `run_prefixflow_step` on
+    every shard fills the full group's bf16 outputs; LSE / gK1 / gV1 are per shard."""
+    if g.Hkv % world != 0:
+        raise ValueError(f"{g.Hkv} KV heads do not shard over {world} ranks")
+    G = g.Hq // g.Hkv
+    kv = slice(rank * (g.Hkv // world), (rank + 1) * (g.Hkv // world))
+    qh = slice(kv.start * G, kv.stop * G)
+    q = lambda t: t[:, qh]
+    k = lambda t: t[:, kv]
+    sh = DeviceGroup(qh.stop - qh.start, kv.stop - kv.start, g.d, g.Lp, list(g.Ls),
+                     q(g.Q1), k(g.K1), k(g.V1), q(g.dO1), [], [], [], [])
+    sh.wave = g.wave
+    sh.packed = []
+    dev = g.Q1.device
+    f32 = torch.float32
+    sh.O1, sh.dQ1, sh.dK1, sh.dV1 = q(g.O1), q(g.dQ1), k(g.dK1), k(g.dV1)
+    sh.LSE1 = torch.empty((sh.Hq, g.Lp), dtype=f32, device=dev)
+    sh.gK1 = torch.empty((g.Lp, sh.Hkv, g.d), dtype=f32, device=dev)
+    sh.gV1 = torch.empty_like(sh.gK1)
+    sh.O2, sh.LSE2, sh.dQ2, sh.dK2, sh.dV2 = [], [], [], [], []
+    max_tok = 0
+    for pk in g.packed:
+        cu = pk["cu"]
+        max_tok = max(max_tok, cu[-1])
+        spk = {"cu": cu, "idx": pk["idx"]}
+        for name in ("Q2", "dO2", "O2", "dQ2"):
+            spk[name] = q(pk[name])
+        for name in ("K2", "V2", "dK2", "dV2"):
+            spk[name] = k(pk[name])
+        spk["LSE2"] = torch.empty((sh.Hq, cu[-1]), dtype=f32, device=dev)
+        for j in range(len(pk["idx"])):
+            sl = slice(cu[j], cu[j + 1])
+            for name in ("Q2", "K2", "V2", "dO2", "O2", "dQ2", "dK2", "dV2"):
+                getattr(sh, name).append(spk[name][sl])
+            sh.LSE2.append(spk["LSE2"][:, sl])
+        sh.packed.append(spk)
+    sh.desc = pf.make_desc(sh.Hq, sh.Hkv, g.d)
+    sh.workspace = torch.empty(pf.pf_workspace_bytes(sh.desc, g.Lp, max_tok), dtype=torch.uint8, device=dev)
+    return sh
+
+
 @dataclasses.dataclass
 class ReplayBuffers:
     """Concatenated [P || S(i)] tensors of the N-times replay baseline (one set per trajectory)."""
@@ -160,244 +207,74 @@ def run_replay_step(ctx, r: ReplayBuffers, stream=None) -> None:
 
 
 # --------------------------------------------------------------------------------------------------
-# Memory lifecycle of one layer: hot set {K1, V1, gK1, gV1} stays resident, the
-# dormant Phase-A set {Q1, O1, LSE1} leaves for pinned host memory on a side stream while Phase B
-# runs and is prefetched back before Phase C; suffix-wave tensors live only during their wave.
+# The same replay with all N full sequences packed into ONE launch pair (Lp = 0, n_seqs = N): the
+# fair "same kernels" baseline when the step under test packs its suffixes too -- both pay one launch
+# tail per kernel.
 # --------------------------------------------------------------------------------------------------
-def run_lifecycle_step(ctx, inp, device="cuda", wave: int = 1, offload: bool = True,
-                       pinned: Optional[dict] = None, keep_outputs: bool = False) -> dict:
-    """One A -> B -> C step that allocates and frees device tensors the way a trainer would.
-    Returns peak allocated bytes of the whole step and of Phase B alone (the paper's
-    "Phase-B peak HBM"), the step time, and (optionally) the outputs."""
-    s = inp.shape
-    dev = torch.device(device)
-    Hq, Hkv, d, Lp = s.n_q_heads, s.n_kv_heads, s.head_dim, s.Lp
-    bf, f32 = torch.bfloat16, torch.float32
-    main = torch.cuda.current_stream(dev)
-    side = pinned.setdefault("side_stream", torch.cuda.Stream(dev)) if pinned is not None else torch.cuda.Stream(dev)
-    pinned = pinned if pinned is not None else {}
+@dataclasses.dataclass
+class PackedReplay:
+    cu: List[int]
+    Q: torch.Tensor; K: torch.Tensor; V: torch.Tensor; dO: torch.Tensor
+    O: torch.Tensor; LSE: torch.Tensor; dQ: torch.Tensor; dK: torch.Tensor; dV: torch.Tensor
+    workspace: torch.Tensor
+    desc: pf.pf_desc
 
-    def pin(name, like):
-        if name not in pinned:
-            pinned[name] = torch.empty(like.shape, dtype=like.dtype, pin_memory=True)
-        return pinned[name]
 
-    e = lambda L, H, dt=bf: torch.empty((L, H, d), dtype=dt, device=dev)
-    waves = _waves(s.N, wave)
-    max_tok = max((sum(s.Ls[k] for k in w) for w in waves), default=0)
-    desc = pf.make_desc(Hq, Hkv, d)
-    torch.cuda.synchronize(dev)
-    torch.cuda.reset_peak_memory_stats(dev)
-    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    t0.record(main)
-    # ---- Phase A
-    Q1, K1, V1 = inp.Q1.to(dev), inp.K1.to(dev), inp.V1.to(dev)
-    O1 = e(Lp, Hq); LSE1 = torch.empty((Hq, Lp), dtype=f32, device=dev)
-    gK1, gV1 = e(Lp, Hkv, f32), e(Lp, Hkv, f32)
-    ws = torch.empty(pf.pf_workspace_bytes(desc, Lp, max_tok), dtype=torch.uint8, device=dev)
-    grp = pf.pf_group_begin(ctx, desc, Lp, K1, V1, gK1, gV1, ws, main)
-    outs = {}
+def make_replay_packed(g: DeviceGroup, prefix_weight: Optional[float] = None) -> PackedReplay:
+    """[P || S(1)] ... [P || S(N)] back to back along the token axis; replay i sees the prefix-row
+    adjoint w_i dO1, w_i = 1/N by default (reading 1; input preparation of the baseline)."""
+    n = len(g.Ls)
+    w = (1.0 / n if n else 1.0) if prefix_weight is None else prefix_weight
+    dO1w = (g.dO1.float() * w).to(torch.bfloat16)
+    cat = lambda first, rest: torch.cat([t for r in rest for t in (first, r)], 0).contiguous()
+    Q, K, V, dO = cat(g.Q1, g.Q2), cat(g.K1, g.K2), cat(g.V1, g.V2), cat(dO1w, g.dO2)
+    cu = [0]
+    for L in g.Ls:
+        cu.append(cu[-1] + g.Lp + L)
+    dev = g.Q1.device
+    e = lambda t: torch.empty_like(t)
+    nbytes = pf.pf_workspace_bytes(g.desc, 0, cu[-1])
+    return PackedReplay(cu, Q, K, V, dO, e(Q), torch.empty((g.Hq, cu[-1]), dtype=torch.float32, device=dev),
+                        e(Q), e(K), e(V), torch.empty(nbytes, dtype=torch.uint8, device=dev), g.desc)
+
+
+def run_replay_packed_step(ctx, r: PackedReplay, stream=None) -> None:
+    """One forward and one backward launch over the N packed full sequences (plain causal attention:
+    a group without a prefix whose `suffixes` are the whole trajectories)."""
+    grp = pf.pf_group_begin(ctx, r.desc, 0, None, None, None, None, r.workspace, stream)
     try:
-        pf.pf_phaseA_fwd(grp, Q1, O1, LSE1, main)
-        dormant = {"Q1": Q1, "O1": O1, "LSE1": LSE1}
-        if offload:
-            evA = torch.cuda.Event(); evA.record(main)
-            side.wait_event(evA)
-            for name, t in dormant.items():
-                pf.pf_offload(ctx, t, pin(name, t), side)
-            side.synchronize()        # the copies ran beside nothing here; a trainer overlaps them with wave 1
-            if keep_outputs:
-                outs["O1"], outs["LSE1"] = O1.clone(), LSE1.clone()
-            shapes = {k: (t.shape, t.dtype) for k, t in dormant.items()}
-            del Q1, O1, LSE1, dormant
-        # ---- Phase B, one wave at a time; a wave's tensors are freed when the wave is done
-        peak_a = torch.cuda.max_memory_allocated(dev)
-        torch.cuda.reset_peak_memory_stats(dev)
-        base = torch.cuda.memory_allocated(dev)
-        for w in waves:
-            cu = [0]
-            for k in w:
-                cu.append(cu[-1] + s.Ls[k])
-            cat = lambda src: torch.cat([src[k] for k in w], 0).contiguous().to(dev)
-            Q2, K2, V2, dO2 = cat(inp.Q2), cat(inp.K2), cat(inp.V2), cat(inp.dO2)
-            tot = cu[-1]
-            O2, dQ2 = e(tot, Hq), e(tot, Hq)
-            dK2, dV2 = e(tot, Hkv), e(tot, Hkv)
-            LSE2 = torch.empty((Hq, tot), dtype=f32, device=dev)
-            pf.pf_phaseB_fwd(grp, cu, Q2, K2, V2, O2, LSE2, main)
-            pf.pf_phaseB_bwd(grp, cu, Q2, K2, V2, O2, LSE2, dO2, dQ2, dK2, dV2, main)
-            if keep_outputs:
-                for j, k in enumerate(w):
-                    sl = slice(cu[j], cu[j + 1])
-                    outs[f"O2[{k}]"], outs[f"LSE2[{k}]"] = O2[sl].clone(), LSE2[:, sl].clone()
-                    outs[f"dQ2[{k}]"], outs[f"dK2[{k}]"], outs[f"dV2[{k}]"] = (
-                        dQ2[sl].clone(), dK2[sl].clone(), dV2[sl].clone())
-            del Q2, K2, V2, dO2, O2, dQ2, dK2, dV2, LSE2
-        peak_b = torch.cuda.max_memory_allocated(dev)
-        # ---- prefetch the dormant set back (side stream), then Phase C
-        if offload:
-            Q1 = torch.empty(shapes["Q1"][0], dtype=shapes["Q1"][1], device=dev)
-            O1 = torch.empty(shapes["O1"][0], dtype=shapes["O1"][1], device=dev)
-            LSE1 = torch.empty(shapes["LSE1"][0], dtype=shapes["LSE1"][1], device=dev)
-            evB = torch.cuda.Event(); evB.record(main)   # the fresh buffers may reuse blocks Phase B still reads
-            side.wait_event(evB)
-            for name, t in (("Q1", Q1), ("O1", O1), ("LSE1", LSE1)):
-                pf.pf_prefetch(ctx, pinned[name], t, side)
-            evP = torch.cuda.Event(); evP.record(side)
-            main.wait_event(evP)
-        elif keep_outputs:
-            outs["O1"], outs["LSE1"] = O1.clone(), LSE1.clone()
-        dO1 = inp.dO1.to(dev)
-        dQ1, dK1, dV1 = e(Lp, Hq), e(Lp, Hkv), e(Lp, Hkv)
-        pf.pf_phaseC_bwd(grp, Q1, O1, LSE1, dO1, dQ1, dK1, dV1, main)
+        pf.pf_group_mark_cached(grp)
+        pf.pf_phaseB_fwd(grp, r.cu, r.Q, r.K, r.V, r.O, r.LSE, stream)
+        pf.pf_phaseB_bwd(grp, r.cu, r.Q, r.K, r.V, r.O, r.LSE, r.dO, r.dQ, r.dK, r.dV, stream)
     finally:
         pf.pf_group_end(grp)
-    t1.record(main)
-    torch.cuda.synchronize(dev)
-    if keep_outputs:
-        outs.update(dQ1=dQ1, dK1=dK1, dV1=dV1)
-    return dict(ms=t0.elapsed_time(t1), peak_step_bytes=max(peak_a, torch.cuda.max_memory_allocated(dev)),
-                peak_phaseB_bytes=peak_b, resident_at_phaseB_start_bytes=base, outputs=outs)
 
 
-# --------------------------------------------------------------------------------------------------
-# Multi-layer lifecycle (SURVEY.md §8f item 2; PAPER.md:232-240, 385): L attention layers, each with
-# its own training-time KV cache.  Phase A runs layer by layer and every layer's dormant set
-# {Q1, O1, LSE1} leaves for the pinned host pool on the side stream as soon as it is produced;
-# Phase B runs all waves on all layers with only the hot sets {K1, V1, gK1, gV1} resident; Phase C
-# runs in reverse layer order with the dormant set of layer l-1 prefetched while layer l computes
-# (if a prefetch has not been issued or has not landed, Phase C simply waits for it: demand load).
-# --------------------------------------------------------------------------------------------------
-def run_multilayer_step(ctx, layers, device="cuda", wave: int = 1, offload: bool = True,
-                        pinned: Optional[dict] = None, keep_outputs: bool = False,
-                        early_prefetch: bool = False) -> dict:
-    """`layers`: list of inputs.GroupInputs with identical shapes (one per attention layer).
-    `early_prefetch` issues the first Phase-C prefetch behind the last Phase-B wave: no exposed wait,
-    but its buffers count in the Phase-B peak."""
-    s = layers[0].shape
+def random_device_group(shape, device="cuda", wave: int = 1, seed: int = 0) -> DeviceGroup:
+    """A rollout group of the given shape drawn directly on the device (N(0,1)/sqrt(d) -> bf16):
+    for timing sweeps over many configurations, where values do not matter and the CPU generator
+    of `inputs.make_group` would dominate the run.  Parity tests never use this."""
     dev = torch.device(device)
-    Hq, Hkv, d, Lp, L = s.n_q_heads, s.n_kv_heads, s.head_dim, s.Lp, len(layers)
-    bf, f32 = torch.bfloat16, torch.float32
-    main = torch.cuda.current_stream(dev)
-    pinned = pinned if pinned is not None else {}
-    side = pinned.setdefault("side_stream", torch.cuda.Stream(dev))
-    e = lambda n, H, dt=bf: torch.empty((n, H, d), dtype=dt, device=dev)
-    waves = _waves(s.N, wave)
-    max_tok = max((sum(s.Ls[k] for k in w) for w in waves), default=0)
-    desc = pf.make_desc(Hq, Hkv, d)
-
-    def pin(l, name, like):
-        key = (l, name)
-        if key not in pinned:
-            pinned[key] = torch.empty(like.shape, dtype=like.dtype, pin_memory=True)
-        return pinned[key]
-
-    torch.cuda.synchronize(dev)
-    torch.cuda.reset_peak_memory_stats(dev)
-    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    t0.record(main)
-    ws = torch.empty(pf.pf_workspace_bytes(desc, Lp, max_tok), dtype=torch.uint8, device=dev)
-    hot, dorm, grp, outs = [], [], [], [dict() for _ in range(L)]
-    exposed = []                                    # (event before wait, event after wait) per layer
-    try:
-        # ---- Phase A, layer by layer; dormant sets stream out behind it
-        for l, inp in enumerate(layers):
-            Q1, K1, V1 = inp.Q1.to(dev), inp.K1.to(dev), inp.V1.to(dev)
-            O1 = e(Lp, Hq); LSE1 = torch.empty((Hq, Lp), dtype=f32, device=dev)
-            gK1, gV1 = e(Lp, Hkv, f32), e(Lp, Hkv, f32)
-            g = pf.pf_group_begin(ctx, desc, Lp, K1, V1, gK1, gV1, ws, main)
-            grp.append(g)
-            pf.pf_phaseA_fwd(g, Q1, O1, LSE1, main)
-            hot.append(dict(K1=K1, V1=V1, gK1=gK1, gV1=gV1))
-            dset = dict(Q1=Q1, O1=O1, LSE1=LSE1)
-            if keep_outputs:
-                outs[l]["O1"], outs[l]["LSE1"] = O1.clone(), LSE1.clone()
-            if offload:
-                ev = torch.cuda.Event(); ev.record(main)
-                side.wait_event(ev)
-                for name, t in dset.items():
-                    pf.pf_offload(ctx, t, pin(l, name, t), side)
-                dset = dict(shapes={k: (t.shape, t.dtype) for k, t in dset.items()},
-                            done=torch.cuda.Event())
-                dset["done"].record(side)
-                dset["keep"] = (Q1, O1, LSE1)       # freed once the copy has left (below)
-            dorm.append(dset)
-            del Q1, O1, LSE1
-        if offload:
-            side.synchronize()                      # all dormant sets are on the host: free them
-            for dset in dorm:
-                dset.pop("keep")
-        peak_a = torch.cuda.max_memory_allocated(dev)
-        torch.cuda.reset_peak_memory_stats(dev)
-        base = torch.cuda.memory_allocated(dev)
-        def prefetch(l):
-            dset = dorm[l]
-            ev = torch.cuda.Event(); ev.record(main)   # fresh buffers may reuse blocks main still reads
-            bufs = {k: torch.empty(sh, dtype=dt, device=dev) for k, (sh, dt) in dset["shapes"].items()}
-            side.wait_event(ev)
-            for name, t in bufs.items():
-                pf.pf_prefetch(ctx, pinned[(l, name)], t, side)
-            dset["bufs"], dset["landed"] = bufs, torch.cuda.Event()
-            dset["landed"].record(side)
-
-        # ---- Phase B: every wave on every layer (a wave's tensors live only during the wave)
-        for wi, w in enumerate(waves):
-            if offload and early_prefetch and wi == len(waves) - 1:
-                prefetch(L - 1)                       # hidden behind the last wave (costs its buffers in the Phase-B peak)
-            cu = [0]
-            for k in w:
-                cu.append(cu[-1] + s.Ls[k])
-            tot = cu[-1]
-            for l, inp in enumerate(layers):
-                cat = lambda src: torch.cat([src[k] for k in w], 0).contiguous().to(dev)
-                Q2, K2, V2, dO2 = cat(inp.Q2), cat(inp.K2), cat(inp.V2), cat(inp.dO2)
-                O2, dQ2, dK2, dV2 = e(tot, Hq), e(tot, Hq), e(tot, Hkv), e(tot, Hkv)
-                LSE2 = torch.empty((Hq, tot), dtype=f32, device=dev)
-                pf.pf_phaseB_fwd(grp[l], cu, Q2, K2, V2, O2, LSE2, main)
-                pf.pf_phaseB_bwd(grp[l], cu, Q2, K2, V2, O2, LSE2, dO2, dQ2, dK2, dV2, main)
-                if keep_outputs:
-                    for j, k in enumerate(w):
-                        sl = slice(cu[j], cu[j + 1])
-                        outs[l][f"O2[{k}]"], outs[l][f"LSE2[{k}]"] = O2[sl].clone(), LSE2[:, sl].clone()
-                        outs[l][f"dQ2[{k}]"], outs[l][f"dK2[{k}]"], outs[l][f"dV2[{k}]"] = (
-                            dQ2[sl].clone(), dK2[sl].clone(), dV2[sl].clone())
-                del Q2, K2, V2, dO2, O2, dQ2, dK2, dV2, LSE2
-        peak_b = torch.cuda.max_memory_allocated(dev)
-
-        # ---- Phase C in reverse layer order, prefetching one layer ahead
-        if offload and "bufs" not in dorm[L - 1]:
-            prefetch(L - 1)
-        for l in range(L - 1, -1, -1):
-            if offload:
-                if "bufs" not in dorm[l]:
-                    prefetch(l)                       # demand load: nobody prefetched this layer
-                b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                b0.record(main)
-                main.wait_event(dorm[l]["landed"])
-                b1.record(main)
-                exposed.append((b0, b1))
-                if l > 0:
-                    prefetch(l - 1)                   # overlaps Phase C of layer l
-                Q1, O1, LSE1 = (dorm[l]["bufs"][k] for k in ("Q1", "O1", "LSE1"))
-            else:
-                Q1, O1, LSE1 = (dorm[l][k] for k in ("Q1", "O1", "LSE1"))
-            dO1 = layers[l].dO1.to(dev)
-            dQ1, dK1, dV1 = e(Lp, Hq), e(Lp, Hkv), e(Lp, Hkv)
-            pf.pf_phaseC_bwd(grp[l], Q1, O1, LSE1, dO1, dQ1, dK1, dV1, main)
-            if keep_outputs:
-                outs[l].update(dQ1=dQ1, dK1=dK1, dV1=dV1)
-            dorm[l] = None
-            hot[l] = None
-            del Q1, O1, LSE1, dO1, dQ1, dK1, dV1
-    finally:
-        for g in grp:
-            pf.pf_group_end(g)
-    t1.record(main)
-    torch.cuda.synchronize(dev)
-    return dict(ms=t0.elapsed_time(t1), layers=L,
-                peak_step_bytes=max(peak_a, peak_b, torch.cuda.max_memory_allocated(dev)),
-                peak_phaseB_bytes=peak_b, resident_at_phaseB_start_bytes=base,
-                exposed_prefetch_ms=sum(a.elapsed_time(b) for a, b in exposed), outputs=outs)
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(seed)
+    d, sc = shape.head_dim, shape.head_dim ** -0.5
+    draw = lambda L, H: (torch.randn((L, H, d), generator=gen, device=dev, dtype=torch.float32) * sc).to(torch.bfloat16)
+    Hq, Hkv = shape.n_q_heads, shape.n_kv_heads
+    g = DeviceGroup(Hq, Hkv, d, shape.Lp, list(shape.Ls), draw(shape.Lp, Hq), draw(shape.Lp, Hkv),
+                    draw(shape.Lp, Hkv), draw(shape.Lp, Hq), [], [], [], [])
+    g.wave = max(1, int(wave))
+    g.packed = []
+    for w in _waves(shape.N, g.wave):
+        cu = [0]
+        for k in w:
+            cu.append(cu[-1] + shape.Ls[k])
+        pk = {"cu": cu, "idx": w}
+        for name, H in (("Q2", Hq), ("K2", Hkv), ("V2", Hkv), ("dO2", Hq)):
+            pk[name] = draw(cu[-1], H)
+            getattr(g, name).extend(pk[name][cu[j]:cu[j + 1]] for j in range(len(w)))
+        g.packed.append(pk)
+    alloc_outputs(g)
+    return g
 
 
 # --------------------------------------------------------------------------------------------------

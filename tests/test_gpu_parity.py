@@ -8,7 +8,7 @@ import torch
 
 import oracle
 from paper_2606_01143_b200 import binding as pf
-from paper_2606_01143_b200 import inputs, schedule
+from paper_2606_01143_b200 import inputs, lifecycle, schedule
 from parity_util import RAMP_RMS_REL, STRICT_RMS_REL, check, compare_group
 
 pytestmark = pytest.mark.gpu
@@ -354,46 +354,135 @@ def test_workspace_error_leaves_accumulators_untouched(ctx):
     pf.pf_group_end(grp)
 
 
-@pytest.mark.parametrize("offload", [False, True])
+def _check_layer(tag, o, ref, N):
+    check(f"{tag} O1", o["O1"], ref.O1); check(f"{tag} LSE1", o["LSE1"], ref.LSE1, lse=True)
+    for i in range(N):
+        check(f"{tag} O2[{i}]", o[f"O2[{i}]"], ref.O2[i])
+        check(f"{tag} LSE2[{i}]", o[f"LSE2[{i}]"], ref.LSE2[i], lse=True)
+        check(f"{tag} dQ2[{i}]", o[f"dQ2[{i}]"], ref.dQ2[i])
+        check(f"{tag} dK2[{i}]", o[f"dK2[{i}]"], ref.dK2[i]); check(f"{tag} dV2[{i}]", o[f"dV2[{i}]"], ref.dV2[i])
+    check(f"{tag} dQ1", o["dQ1"], ref.dQ1); check(f"{tag} dK1", o["dK1"], ref.dK1); check(f"{tag} dV1", o["dV1"], ref.dV1)
+
+
+@pytest.mark.parametrize("offload", ["none", "wait", "overlap"])
 def test_memory_lifecycle_offload(ctx, offload):
-    """the dormant Phase-A set {Q1, O1, LSE1} moved to pinned host memory during
-    Phase B and prefetched back for Phase C changes no result, and lowers the Phase-B peak."""
+    """the dormant Phase-A set {Q1, O1, LSE1} moved to a pinned host pool behind
+    Phase A and prefetched back for Phase C changes no result; when Phase B waits for the copy it
+    runs with less HBM (with "overlap" it never waits and frees the set when the copy is seen done)."""
     shape = inputs.small_case(4, 2, 128, 700, [130, 64, 200], seed=41, dist="unit")
     inp = inputs.make_group(shape)
     ref = oracle.group_reference(inp)
-    r = schedule.run_lifecycle_step(ctx, inp, wave=2, offload=offload, keep_outputs=True)
-    o = r["outputs"]
-    check("O1", o["O1"], ref.O1); check("LSE1", o["LSE1"], ref.LSE1, lse=True)
-    for i in range(shape.N):
-        check(f"O2[{i}]", o[f"O2[{i}]"], ref.O2[i]); check(f"LSE2[{i}]", o[f"LSE2[{i}]"], ref.LSE2[i], lse=True)
-        check(f"dQ2[{i}]", o[f"dQ2[{i}]"], ref.dQ2[i])
-        check(f"dK2[{i}]", o[f"dK2[{i}]"], ref.dK2[i]); check(f"dV2[{i}]", o[f"dV2[{i}]"], ref.dV2[i])
-    check("dQ1", o["dQ1"], ref.dQ1); check("dK1", o["dK1"], ref.dK1); check("dV1", o["dV1"], ref.dV1)
-    if offload:
-        base = schedule.run_lifecycle_step(ctx, inp, wave=2, offload=False)
+    pool = lifecycle.PinnedPool(int(1.5 * lifecycle.dormant_bytes(shape)))
+    r = lifecycle.run_layers(ctx, lifecycle.HostSource([inp], "cuda"), wave=2, offload=offload, pool=pool,
+                             keep_outputs=True)
+    _check_layer("L0", r["outputs"][0], ref, shape.N)
+    assert r["kept_resident_bytes"] == 0
+    if offload == "wait":
+        base = lifecycle.run_layers(ctx, lifecycle.HostSource([inp], "cuda"), wave=2, offload="none")
         assert r["resident_at_phaseB_start_bytes"] < base["resident_at_phaseB_start_bytes"]
         assert r["peak_phaseB_bytes"] < base["peak_phaseB_bytes"]
+        assert 0 < r["pool_high_water_bytes"] <= r["pool_bytes"]
 
 
-@pytest.mark.parametrize("offload", [False, True])
+@pytest.mark.parametrize("offload", ["none", "wait", "overlap"])
 def test_multilayer_offload_pipeline(ctx, offload):
-    """L layers of caches, dormant sets offloaded as produced, Phase C in reverse
-    layer order with one-layer-ahead prefetch.  Every layer must still match its oracle."""
+    """L layers of caches, dormant sets offloaded as produced, Phase C in
+    reverse layer order with one-layer-ahead prefetch.  Every layer must still match its oracle."""
     shapes = [inputs.small_case(4, 2, 128, 300, [130, 64, 70], seed=50 + l, dist="unit") for l in range(3)]
     layers = [inputs.make_group(s) for s in shapes]
-    r = schedule.run_multilayer_step(ctx, layers, wave=2, offload=offload, keep_outputs=True)
+    pool = lifecycle.PinnedPool(int(1.5 * 3 * lifecycle.dormant_bytes(shapes[0])))
+    r = lifecycle.run_layers(ctx, lifecycle.HostSource(layers, "cuda"), wave=2, offload=offload, pool=pool,
+                             keep_outputs=True, early_prefetch=(offload == "overlap"))
     for l, inp in enumerate(layers):
-        ref = oracle.group_reference(inp)
-        o = r["outputs"][l]
-        check(f"L{l} O1", o["O1"], ref.O1); check(f"L{l} LSE1", o["LSE1"], ref.LSE1, lse=True)
-        for i in range(shapes[l].N):
-            check(f"L{l} O2[{i}]", o[f"O2[{i}]"], ref.O2[i])
-            check(f"L{l} dQ2[{i}]", o[f"dQ2[{i}]"], ref.dQ2[i])
-            check(f"L{l} dK2[{i}]", o[f"dK2[{i}]"], ref.dK2[i]); check(f"L{l} dV2[{i}]", o[f"dV2[{i}]"], ref.dV2[i])
-        check(f"L{l} dQ1", o["dQ1"], ref.dQ1); check(f"L{l} dK1", o["dK1"], ref.dK1); check(f"L{l} dV1", o["dV1"], ref.dV1)
-    if offload:
-        base = schedule.run_multilayer_step(ctx, layers, wave=2, offload=False)
+        _check_layer(f"L{l}", r["outputs"][l], oracle.group_reference(inp), shapes[l].N)
+    if offload == "wait":
+        base = lifecycle.run_layers(ctx, lifecycle.HostSource(layers, "cuda"), wave=2, offload="none")
         assert r["peak_phaseB_bytes"] < base["peak_phaseB_bytes"]
+
+
+def test_offload_fallbacks(ctx):
+    """a pool too small for a layer's dormant set leaves that set in HBM, and a prefetch
+    that does not fit the HBM headroom becomes a demand load -- results never depend on either."""
+    shapes = [inputs.small_case(4, 2, 128, 300, [130, 64], seed=80 + l, dist="unit") for l in range(3)]
+    layers = [inputs.make_group(s) for s in shapes]
+    pool = lifecycle.PinnedPool(int(2.2 * lifecycle.dormant_bytes(shapes[0])))      # room for two of three
+    r = lifecycle.run_layers(ctx, lifecycle.HostSource(layers, "cuda"), wave=1, offload="wait", pool=pool,
+                             keep_outputs=True, hbm_headroom_bytes=1 << 60)         # no early prefetch fits
+    for l, inp in enumerate(layers):
+        _check_layer(f"L{l}", r["outputs"][l], oracle.group_reference(inp), shapes[l].N)
+    assert r["kept_resident_bytes"] == lifecycle.dormant_bytes(shapes[0])
+    assert r["demand_loads"] == 2                                                   # the two offloaded layers
+
+
+def test_deterministic_gkv_is_bit_reproducible(ctx):
+    """Option "deterministic_gkv": one CTA per key tile, one add per accumulator tile and launch --
+    the fp32 gK1 / gV1 (and bf16 dK / dV) of two runs are bit-identical, and still match the oracle."""
+    shape = inputs.small_case(7, 1, 128, 700, [300, 140, 65], seed=95, dist="unit")
+    inp = inputs.make_group(shape)
+    ref = oracle.group_reference(inp)
+    pf.pf_set_option(ctx, "deterministic_gkv", 1)
+    try:
+        runs = []
+        for _ in range(2):
+            g = schedule.to_device(inp, wave=3)
+            snaps = {}
+            schedule.run_prefixflow_step(ctx, g, after_each_suffix=lambda i: snaps.update(
+                {i: (g.gK1.clone(), g.gV1.clone())}))
+            torch.cuda.synchronize()
+            compare_group(g, ref, snaps)
+            runs.append((snaps[2][0], snaps[2][1], g.dK1.clone(), g.dV1.clone(), g.dK2[0].clone()))
+        for a, b in zip(*runs):
+            assert torch.equal(a, b)
+    finally:
+        pf.pf_set_option(ctx, "deterministic_gkv", 0)
+
+
+def test_kv_head_sharding_equals_unsharded(ctx):
+    """SURVEY.md section 8e(i) / PAPER.md:248-252: every phase of ONE group run per KV-head shard on
+    head slices in place (no communication) reproduces the unsharded result and the oracle."""
+    shape = inputs.small_case(8, 4, 128, 300, [129, 64, 200], seed=91, dist="unit")
+    inp = inputs.make_group(shape)
+    ref = oracle.group_reference(inp)
+    g = schedule.to_device(inp, wave=3)
+    shards = [schedule.head_shard(g, 2, r) for r in range(2)]
+    for sh in shards:
+        schedule.run_prefixflow_step(ctx, sh)
+    torch.cuda.synchronize()
+    g.LSE1 = torch.cat([sh.LSE1 for sh in shards], 0)
+    g.LSE2 = [torch.cat([sh.LSE2[i] for sh in shards], 0) for i in range(shape.N)]
+    compare_group(g, ref)                                     # the bf16 outputs were written in place
+    gk = torch.cat([sh.gK1 for sh in shards], 1)              # after Phase C: own-prefix term + coupling
+    check("gK1 (own + coupling, fp32)", gk, ref.dK1)
+
+
+@pytest.mark.parametrize("world,wave", [(2, 0), (4, 1)])
+def test_split_group_schedule_on_one_gpu(ctx, world, wave):
+    """SURVEY.md section 8f item 3 / PAPER.md:270-276, 284-286: head-sharded Phase A, all-gather of
+    K1/V1, Phase B of each rank's suffixes on all heads into a local fp32 gK1/gV1, reduce-scatter over
+    the KV-head dimension, head-sharded Phase C -- the exact per-rank calls, run rank after rank on
+    one GPU with the collectives done in-process (dist.LocalComm)."""
+    from paper_2606_01143_b200 import dist as pfd
+    shape = inputs.small_case(8, 4, 128, 300, [129, 64, 200, 70, 33], seed=93, dist="unit")
+    inp = inputs.make_group(shape)
+    ref = oracle.group_reference(inp)
+    ranks = pfd.run_split_group_local(ctx, inp, world, wave=wave)
+    torch.cuda.synchronize()
+    cat = lambda name, dim: torch.cat([getattr(r, name) for r in ranks], dim)
+    check("O1", cat("O1", 1), ref.O1); check("LSE1", cat("LSE1", 0), ref.LSE1, lse=True)
+    check("dQ1", cat("dQ1", 1), ref.dQ1); check("dK1", cat("dK1", 1), ref.dK1); check("dV1", cat("dV1", 1), ref.dV1)
+    seen = []
+    for r in ranks:
+        for pk in r.pk:
+            for j, i in enumerate(pk["idx"]):
+                sl = slice(pk["cu"][j], pk["cu"][j + 1])
+                seen.append(i)
+                check(f"O2[{i}]", pk["O2"][sl], ref.O2[i]); check(f"LSE2[{i}]", pk["LSE2"][:, sl], ref.LSE2[i], lse=True)
+                check(f"dQ2[{i}]", pk["dQ2"][sl], ref.dQ2[i])
+                check(f"dK2[{i}]", pk["dK2"][sl], ref.dK2[i]); check(f"dV2[{i}]", pk["dV2"][sl], ref.dV2[i])
+        # the rank's local accumulator = the sum of ITS suffixes' coupling gradients, all heads
+        want = sum(ref.gK1_each[i] for i in r.plan.suffixes) if r.plan.suffixes else np.zeros_like(ref.gK1_each[0])
+        check(f"rank {r.plan.rank} local gK1", r.gK1f, want)
+    assert sorted(seen) == list(range(shape.N))               # every suffix ran on exactly one rank
 
 
 @pytest.mark.parametrize("Hq,Hkv,d,segs", [
