@@ -67,7 +67,7 @@ struct pf_group {
     pf::PrefixRanges pre;  // visible ranges of the prefix source (default: [0, Lp))
     int state;  // 0 begun, 1 A done, 2 C done
     // descriptor cache: the tensor maps of the borrowed cache tensors are encoded once per group
-    KvMaps kv64, kv128;    // K1/V1 with 64-row boxes (forward) and 128-row boxes (backward)
+    KvMaps kv128;          // K1/V1 with 128-row boxes (both attention kernels)
     KvMaps acc;            // gK1 / gV1 reduce-add maps (valid when gK1 != NULL)
 };
 
@@ -261,7 +261,6 @@ pf::PrefixRanges whole_prefix(int64_t Lp) {
         r.n = 1;
         r.len[0] = int(Lp);
         r.tile0[1] = int((Lp + 127) / 128);
-        r.sub0[1] = int((Lp + 63) / 64);
     }
     return r;
 }
@@ -295,8 +294,8 @@ pf_status launch_fwd(pf_group* g, const pf_tensor& Q, const KvMaps* prefix, int6
     KvMaps own;
     pf_status st;
     if (!causal) {
-        if ((st = make_map(ctx, &own.k, "K", K2, total, Hkv, D, 64))) return st;
-        if ((st = make_map(ctx, &own.v, "V", V2, total, Hkv, D, 64))) return st;
+        if ((st = make_map(ctx, &own.k, "K", K2, total, Hkv, D))) return st;
+        if ((st = make_map(ctx, &own.v, "V", V2, total, Hkv, D))) return st;
         causal = &own;
     }
     if (Lp == 0 || !prefix) prefix = causal;
@@ -655,8 +654,7 @@ pf_status pf_group_begin(pf_ctx* ctx, const pf_desc* desc, int64_t Lp, pf_tensor
     g->state = 0;
     if (Lp > 0) {
         pf_status ms;
-        if ((ms = make_map(ctx, &g->kv64.k, "K1", K1, Lp, Hkv, d, 64)) || (ms = make_map(ctx, &g->kv64.v, "V1", V1, Lp, Hkv, d, 64)) ||
-            (ms = make_map(ctx, &g->kv128.k, "K1", K1, Lp, Hkv, d, 128)) || (ms = make_map(ctx, &g->kv128.v, "V1", V1, Lp, Hkv, d, 128)) ||
+        if ((ms = make_map(ctx, &g->kv128.k, "K1", K1, Lp, Hkv, d, 128)) || (ms = make_map(ctx, &g->kv128.v, "V1", V1, Lp, Hkv, d, 128)) ||
             (ms = make_acc_map(ctx, &g->acc.k, "gK1", g->gK1, Lp, Hkv, d)) || (ms = make_acc_map(ctx, &g->acc.v, "gV1", g->gV1, Lp, Hkv, d))) {
             delete g;
             return ms;
@@ -696,8 +694,8 @@ pf_status pf_phaseA_fwd(pf_group* grp, pf_tensor Q1, pf_tensor O1, float* LSE1, 
     if (Lp > 0) {
         cudaStream_t s = static_cast<cudaStream_t>(stream);
         const int64_t cu[2] = {0, Lp};
-        st = d == 64 ? launch_fwd<64>(grp, Q1, nullptr, 0, &grp->kv64, grp->K1, grp->V1, O1, LSE1, Lp, 1, cu, 0, s)
-                     : launch_fwd<128>(grp, Q1, nullptr, 0, &grp->kv64, grp->K1, grp->V1, O1, LSE1, Lp, 1, cu, 0, s);
+        st = d == 64 ? launch_fwd<64>(grp, Q1, nullptr, 0, &grp->kv128, grp->K1, grp->V1, O1, LSE1, Lp, 1, cu, 0, s)
+                     : launch_fwd<128>(grp, Q1, nullptr, 0, &grp->kv128, grp->K1, grp->V1, O1, LSE1, Lp, 1, cu, 0, s);
         if (st) return st;
     }
     grp->state = 1;
@@ -735,8 +733,8 @@ pf_status pf_phaseB_fwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens
         if (n == 0) break;
         const pf_tensor q = tok_offset(Q2, t0), k = tok_offset(K2, t0), v = tok_offset(V2, t0),
                         o = tok_offset(O2, t0);
-        st = d == 64 ? launch_fwd<64>(grp, q, &grp->kv64, grp->Lp, nullptr, k, v, o, LSE2 + t0, total, n, cu, 1, s)
-                     : launch_fwd<128>(grp, q, &grp->kv64, grp->Lp, nullptr, k, v, o, LSE2 + t0, total, n, cu, 1, s);
+        st = d == 64 ? launch_fwd<64>(grp, q, &grp->kv128, grp->Lp, nullptr, k, v, o, LSE2 + t0, total, n, cu, 1, s)
+                     : launch_fwd<128>(grp, q, &grp->kv128, grp->Lp, nullptr, k, v, o, LSE2 + t0, total, n, cu, 1, s);
         if (st) return st;
     }
     return PF_OK;
@@ -833,7 +831,6 @@ pf_status pf_group_set_prefix_ranges(pf_group* grp, int32_t n_ranges, const int6
         r.start[r.n] = int(starts_host[i]);
         r.len[r.n] = int(lens_host[i]);
         r.tile0[r.n + 1] = r.tile0[r.n] + int((lens_host[i] + 127) / 128);
-        r.sub0[r.n + 1] = r.sub0[r.n] + int((lens_host[i] + 63) / 64);
         end = starts_host[i] + lens_host[i];
         ++r.n;
     }

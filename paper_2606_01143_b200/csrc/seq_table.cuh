@@ -22,8 +22,7 @@ struct PrefixRanges {
     int n;
     int start[kMaxRanges];      // first row of range r
     int len[kMaxRanges];        // rows of range r
-    int tile0[kMaxRanges + 1];  // prefix sums of ceil(len / 128): first 128-row tile of range r (backward)
-    int sub0[kMaxRanges + 1];   // prefix sums of ceil(len / 64): first 64-row sub-tile of range r (forward)
+    int tile0[kMaxRanges + 1];  // prefix sums of ceil(len / 128): first 128-row tile of range r
     // tile index -> (range, first row of the tile in the buffer, valid rows of the tile)
     __host__ __device__ void locate(int tile, int& row0, int& valid) const {
         int r = 0;
@@ -31,13 +30,6 @@ struct PrefixRanges {
         const int i = tile - tile0[r];
         row0 = start[r] + i * 128;
         valid = len[r] - i * 128;
-    }
-    __host__ __device__ void locate64(int sub, int& row0, int& valid) const {
-        int r = 0;
-        while (r + 1 < n && sub0[r + 1] <= sub) ++r;
-        const int i = sub - sub0[r];
-        row0 = start[r] + i * 64;
-        valid = len[r] - i * 64;
     }
 };
 
