@@ -104,8 +104,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
     uint64_t* bar_P = bars + 15;            // [2 buffers][2 halves] P half ready (softmax -> MMA)
     uint64_t* bar_PV = bars + 19;           // P.V of an iteration complete (needed before O is rescaled)
     uint64_t* bar_done = bars + 20;         // all MMAs complete
-    uint64_t* bar_X = bars + 21;            // [4] row-max exchange of one row quarter (its four warps)
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 26);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 22);
 
     const int tid = threadIdx.x, warp = tid >> 5;
     if ((smem_u32(smem) & 1023u) != 0) __trap();
@@ -134,7 +133,6 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
         for (int i = 0; i < 4; ++i) mbar_init(&bar_P[i], 256);
         mbar_init(bar_PV, 1);
         mbar_init(bar_done, 1);
-        for (int i = 0; i < 4; ++i) mbar_init(&bar_X[i], 128);
         fence_mbar_init();
     }
     if (warp == 16) {
@@ -261,14 +259,11 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
                 p.pre.locate(it, row0, limit);
             }
             limit -= qd * 32;
-            auto mask_tail = [&]() {             // ragged prefix tail or causal diagonal
-                if (limit < 32) {
+            if (limit < 32) {                    // ragged prefix tail or causal diagonal
 #pragma unroll
-                    for (int j = 0; j < 32; ++j)
-                        if (j >= limit) x[j] = 0xf149f2cau;  // -1e30: exp2 -> 0, stays finite
-                }
-            };
-            mask_tail();
+                for (int j = 0; j < 32; ++j)
+                    if (j >= limit) x[j] = 0xf149f2cau;  // -1e30: exp2 -> 0, stays finite
+            }
             float mx0 = -INFINITY, mx1 = -INFINITY;
 #pragma unroll
             for (int j = 0; j < 32; j += 2) {
@@ -278,62 +273,45 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
             float* xm = xch + b * 512;
             float mine = fmaxf(mx0, mx1);
             xm[qd * 128 + r] = mine;
-            mbar_arrive(&bar_X[warp & 3]);       // published; nobody waits here
-            // ---- P = exp2(c S - m), packed to bf16 (first 16 columns of this quarter of S)
-            float2 sum2;
-            uint32_t pk[16];
-            auto exp_block = [&](float m_ref) {
-                const float2 c2 = make_float2(c, c), nm2 = make_float2(-m_ref, -m_ref);
-                sum2 = make_float2(0.f, 0.f);
-#pragma unroll
-                for (int j = 0; j < 16; ++j) {
-                    const float2 a = __ffma2_rn(make_float2(__uint_as_float(x[2 * j]),
-                                                            __uint_as_float(x[2 * j + 1])), c2, nm2);
-                    float2 e;
-                    if ((j * C::POLY16) % 16 < C::POLY16) {   // POLY16 pairs in 16 on the FMA pipe
-                        e = exp2_poly2(a);
-                    } else {
-                        e.x = fast_exp2(a.x);
-                        e.y = fast_exp2(a.y);
-                    }
-                    sum2 = __fadd2_rn(sum2, e);
-                    pk[j] = pack_bf16(e.x, e.y);
-                }
-            };
-            // Speculation: the reference m_used stays valid while the tile's row maximum is within 2^8
-            // of it, which is the case for all but a handful of (row, tile) events -- so the
-            // exponentials are computed against it BEFORE the other three column quarters' maxima are
-            // known.  The exchange (shared memory + an mbarrier of the row quarter's four warps) then
-            // costs no waiting, and the four warps of a scheduler drift out of phase, so that one
-            // warp's MUFU-bound exponentials overlap another's load / max / store phases.
-            if (it > 0) exp_block(m_used);
-            mbar_wait(&bar_X[warp & 3], it & 1);
+            named_bar_sync(1 + (warp & 3), 128);              // the row quarter's four warps (one per column quarter)
 #pragma unroll
             for (int o = 1; o < 4; ++o) mine = fmaxf(mine, xm[((qd + o) & 3) * 128 + r]);
             const float m_new = mine * c;
             // lazy rescale: keep a stale max while the new one is within 2^8 of it
             const bool need = (it == 0) || (m_new > m_used + 8.f);
-            if (__any_sync(0xffffffffu, need)) {     // slow path: re-reference, then redo this tile's P
-                if (it > 0) {
-                    const unsigned rescale_mask = __ballot_sync(0xffffffffu, need);
-                    if ((tid & 31) == 0 && qd == 0)   // one of the row's four threads counts it
-                        atomicAdd(&g_fwd_rescale_rows, (unsigned long long)__popc(rescale_mask));
-                    mbar_wait(bar_PV, (it - 1) & 1); // P.V(it-1) must have landed in O
-                    tc_fence_after();
-                    const float alpha = need ? fast_exp2(m_used - m_new) : 1.f;
-                    l *= alpha;
-                    uint32_t o[DQ];
-                    if constexpr (D == 128) tmem_ld32(tO, o); else tmem_ld16(tO, o);
-                    tmem_wait_ld();
-#pragma unroll
-                    for (int j = 0; j < DQ; ++j) o[j] = __float_as_uint(__uint_as_float(o[j]) * alpha);
-                    if constexpr (D == 128) tmem_st32(tO, o); else tmem_st16(tO, o);
-                }
-                if (need) m_used = m_new;
-                tmem_ld32(tS, x);                    // S(it) is still in TMEM: P has not been stored yet
+            const unsigned rescale_mask = __ballot_sync(0xffffffffu, need && it > 0);
+            if (rescale_mask != 0u) {
+                if ((tid & 31) == 0 && qd == 0)   // one of the row's four threads counts it
+                    atomicAdd(&g_fwd_rescale_rows, (unsigned long long)__popc(rescale_mask));
+                mbar_wait(bar_PV, (it - 1) & 1); // P.V(it-1) must have landed in O
+                tc_fence_after();
+                const float alpha = need ? fast_exp2(m_used - m_new) : 1.f;
+                l *= alpha;
+                uint32_t o[DQ];
+                if constexpr (D == 128) tmem_ld32(tO, o); else tmem_ld16(tO, o);
                 tmem_wait_ld();
-                mask_tail();
-                exp_block(m_used);
+#pragma unroll
+                for (int j = 0; j < DQ; ++j) o[j] = __float_as_uint(__uint_as_float(o[j]) * alpha);
+                if constexpr (D == 128) tmem_st32(tO, o); else tmem_st16(tO, o);
+            }
+            if (need) m_used = m_new;
+            // ---- P = exp2(c S - m), packed to bf16 over the first 16 columns of this quarter of S
+            const float2 c2 = make_float2(c, c), nm2 = make_float2(-m_used, -m_used);
+            float2 sum2 = make_float2(0.f, 0.f);
+            uint32_t pk[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) {
+                const float2 a = __ffma2_rn(make_float2(__uint_as_float(x[2 * j]),
+                                                        __uint_as_float(x[2 * j + 1])), c2, nm2);
+                float2 e;
+                if ((j * C::POLY16) % 16 < C::POLY16) {   // POLY16 pairs in 16 on the FMA pipe
+                    e = exp2_poly2(a);
+                } else {
+                    e.x = fast_exp2(a.x);
+                    e.y = fast_exp2(a.y);
+                }
+                sum2 = __fadd2_rn(sum2, e);
+                pk[j] = pack_bf16(e.x, e.y);
             }
             tmem_st16(tS, pk);
             tmem_wait_st();
