@@ -295,7 +295,7 @@ def sweep_legs(ctx, schedule, lifecycle, inputs, dev, stream, peaks, steps: int 
                          speedup=ms_r / ms, ideal_speedup_pair_model=F["ideal_speedup"])
         del g, rp
         torch.cuda.empty_cache()
-    m = memory_legs(ctx, lifecycle, inputs.config_32k(), dev, 1, 0, reps=1)
+    m = memory_legs(ctx, lifecycle, inputs.config_32k(), dev, 1, 0, reps=2)
     out["32k"]["memory_single_layer"] = m["single_layer"]
     return out
 
