@@ -372,6 +372,7 @@ def main() -> None:
                     help="suffixes packed per Phase-B call (PAPER.md:158, 242 suffix microbatch); "
                          "0 = all N in one wave (default), 1 = one call per suffix")
     ap.add_argument("--no-wave1", action="store_true", help="skip the extra wave = 1 measurement")
+    ap.add_argument("--no-graph", action="store_true", help="skip the CUDA-graph replay of the step")
     ap.add_argument("--no-offload", action="store_true", help="skip the memory-lifecycle / offload measurement")
     ap.add_argument("--offload-wave", type=int, default=1, help="suffixes per wave in the lifecycle measurement")
     ap.add_argument("--layers", type=int, default=4, help="attention layers in the multi-layer offload pipeline (0 = skip)")
@@ -560,6 +561,27 @@ def main() -> None:
         del g1
         torch.cuda.empty_cache()
 
+    # ---- the same step replayed from a CUDA graph (one launch per step: no gaps between the
+    # dependent memsets / kernels); packed wave and, if measured above, one call per suffix ----
+    graph = None
+    if not args.no_graph:
+        gr = schedule.capture_step(ctx, g)
+        for _ in range(2):
+            gr.replay()
+        ms_g = timed(gr.replay, args.steps)
+        graph = dict(ms_per_step=ms_g, tflops=world * F["step"] / (ms_g * 1e-3) / 1e12, speedup_vs_eager=ms_step / ms_g)
+        del gr
+        if wave1 is not None:
+            g1 = schedule.to_device(inp, dev, wave=1)
+            gr1 = schedule.capture_step(ctx, g1)
+            for _ in range(2):
+                gr1.replay()
+            ms_g1 = timed(gr1.replay, args.steps)
+            graph["wave1_ms_per_step"] = ms_g1
+            graph["wave1_speedup_vs_eager"] = wave1["ms_per_step"] / ms_g1
+            del gr1, g1
+        torch.cuda.empty_cache()
+
     # ---- memory lifecycle: Phase-B peak HBM with the dormant Phase-A set
     # {Q1, O1, LSE1} resident vs offloaded to a pinned host pool on a side stream ----
     memory = None
@@ -680,7 +702,7 @@ def main() -> None:
         metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
         ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="bf16",
         data="synthetic", config=cfg, clocks=clk.summary(), e2e=e2e, gpu_launches=launches,
-        roofline=roofline, roofline_fwd=roofline_fwd, cpu_baseline=cpu, sweep=sweep,
+        roofline=roofline, roofline_fwd=roofline_fwd, cpu_baseline=cpu, sweep=sweep, graph=graph,
         phases=phases, phaseB=dict(ms=b_ms, tflops=phaseB_tflops,
                                    pct_of_bf16_burst=100 * phaseB_tflops / peaks["burst"] if phaseB_tflops else None,
                                    pct_of_bf16_sustained=100 * phaseB_tflops / peaks["sustained"] if phaseB_tflops else None,

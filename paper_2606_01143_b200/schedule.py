@@ -119,6 +119,23 @@ def run_prefixflow_step(ctx, g: DeviceGroup, stream=None, after_each_suffix=None
         pf.pf_group_end(grp)
 
 
+def capture_step(ctx, g: DeviceGroup, order: Optional[Sequence[int]] = None) -> "torch.cuda.CUDAGraph":
+    """One A -> B -> C step captured into a CUDA graph.  Every C-ABI call only enqueues memsets and
+    kernels on the caller's stream (tensor maps and kernel parameters are baked in at capture), so a
+    training loop whose buffers keep their addresses replays the whole step with one launch; the
+    launch gaps between the ~18 (one packed wave) to ~60 (one call per suffix) dependent kernels of
+    a step go away.  The profile option must be off during capture."""
+    side = torch.cuda.Stream(g.Q1.device)
+    side.wait_stream(torch.cuda.current_stream(g.Q1.device))
+    with torch.cuda.stream(side):                 # warm-up outside the capture (lazy module loads)
+        run_prefixflow_step(ctx, g, side, order=order)
+    torch.cuda.current_stream(g.Q1.device).wait_stream(side)
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        run_prefixflow_step(ctx, g, torch.cuda.current_stream(g.Q1.device), order=order)
+    return graph
+
+
 def head_shard(g: DeviceGroup, world: int, rank: int) -> DeviceGroup:
     """KV-head shard `rank` of `world` of a device group (the paper's TP rule: each
     rank caches its own head shard, no communication): the bf16 inputs and outputs are head slices

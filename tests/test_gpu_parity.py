@@ -245,6 +245,24 @@ def test_replay_baseline_matches_oracle(ctx):
         check(f"replay dV[{i}]", r.dV[i], dv)
 
 
+@pytest.mark.parametrize("wave", [0, 1])
+def test_cuda_graph_replay_matches_oracle(ctx, wave):
+    """schedule.capture_step: the whole A -> B -> C step captured into a CUDA graph; outputs are
+    cleared between replays, so what is compared was produced by the replay alone."""
+    shape = inputs.small_case(4, 2, 128, 300, [129, 64, 200], seed=23, dist="unit")
+    inp = inputs.make_group(shape)
+    ref = oracle.group_reference(inp)
+    g = schedule.to_device(inp, wave=wave if wave else shape.N)
+    graph = schedule.capture_step(ctx, g)
+    for _ in range(2):
+        for t in [g.O1, g.LSE1, g.dQ1, g.dK1, g.dV1, g.gK1, g.gV1] + [pk[k] for pk in g.packed
+                                                                     for k in ("O2", "LSE2", "dQ2", "dK2", "dV2")]:
+            t.fill_(float("nan"))
+        graph.replay()
+        torch.cuda.synchronize()
+        compare_group(g, ref)
+
+
 def test_two_groups_on_two_streams(ctx):
     """No hidden shared state: two groups interleaved on two streams both match."""
     shapes = [inputs.small_case(2, 1, 64, 150, [60], seed=31), inputs.small_case(4, 4, 128, 90, [140], seed=32)]
