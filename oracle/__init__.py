@@ -8,3 +8,4 @@ from .reference import (  # noqa: F401
     build, lib, max_threads, widen, fullseq, rows, cols, group_reference, GroupReference,
     sampled_phaseB, sampled_rows,
 )
+from .companions import rope, kv_proj_grad  # noqa: F401

@@ -336,3 +336,65 @@ def test_sampled_helpers_agree_with_full():
     assert np.abs(s["dk2"] - ref.dK2[1][[0, 5], 1]).max() < 1e-13
     assert np.abs(s["o2"] - ref.O2[1][:, 2:4].transpose(1, 0, 2)).max() < 1e-13
     assert np.abs(s["dq2"] - ref.dQ2[1][:, 2:4].transpose(1, 0, 2)).max() < 1e-13
+
+
+# ---------------------------------------------------------------------------------------------
+# companions: RoPE with continuing positions and the dW_K split
+# ---------------------------------------------------------------------------------------------
+
+def test_rope_pins():
+    rng = np.random.default_rng(5)
+    L, H, d, base = 9, 3, 16, 10000.0
+    x = rng.standard_normal((L, H, d))
+    pos = np.arange(100, 100 + L)
+    y = oracle.rope(x, pos, base)
+    # (a) a worked value (tests/golden/rope_worked.txt): d = 2, position 1: the pair is rotated by 1 rad
+    g = oracle.rope(np.array([[[1.0, 0.0]]]), [1], base)
+    assert abs(g[0, 0, 0] - 0.5403023058681398) < 1e-15 and abs(g[0, 0, 1] - 0.8414709848078965) < 1e-15
+    g = oracle.rope(np.array([[[0.0, 1.0]]]), [1], base)      # sign of the cross terms
+    assert abs(g[0, 0, 0] + 0.8414709848078965) < 1e-15 and abs(g[0, 0, 1] - 0.5403023058681398) < 1e-15
+    # (b) position 0 is the identity; rotations preserve the norm of every (token, head) row
+    assert np.abs(oracle.rope(x, np.zeros(L, dtype=int), base) - x).max() == 0.0
+    assert np.abs(np.linalg.norm(y, axis=-1) - np.linalg.norm(x, axis=-1)).max() < 1e-13
+    # (c) independent route: pair (x_j, x_{j+d/2}) as a complex number times e^{i a}; the frequency of
+    # pair j is base^(-2j/d): pair 0 turns by `position` radians, the last pair slowest
+    z = (x[..., : d // 2] + 1j * x[..., d // 2:]) * np.exp(
+        1j * pos[:, None, None] * base ** (-np.arange(d // 2) / (d // 2)))
+    assert np.abs(np.concatenate([z.real, z.imag], -1) - y).max() < 1e-12
+    # (d) the relative-position property that makes continuing positions matter:
+    # <R_m q, R_n k> depends on m - n only, and differs if the suffix restarted at 0
+    q, k = rng.standard_normal((1, 1, d)), rng.standard_normal((1, 1, d))
+    dot = lambda m, n: float((oracle.rope(q, [m], base) * oracle.rope(k, [n], base)).sum())
+    assert abs(dot(1000, 993) - dot(7, 0)) < 1e-11 and abs(dot(1000, 993) - dot(0, 993)) > 1e-3
+    # (e) inverse is the transpose: R^T R = I and <R x, g> = <x, R^T g> (the backward of a linear map)
+    gy = rng.standard_normal((L, H, d))
+    assert np.abs(oracle.rope(y, pos, base, inverse=True) - x).max() < 1e-13
+    assert abs((y * gy).sum() - (x * oracle.rope(gy, pos, base, inverse=True)).sum()) < 1e-11
+    # (f) torch, rotate-half formulation in fp64 (how the HF Llama / Qwen code applies it)
+    xt = torch.tensor(x)
+    inv = base ** (-torch.arange(0, d, 2, dtype=torch.float64) / d)
+    ang = torch.tensor(pos, dtype=torch.float64)[:, None] * inv[None]
+    cos, sin = torch.cat([ang.cos(), ang.cos()], -1)[:, None], torch.cat([ang.sin(), ang.sin()], -1)[:, None]
+    rot = torch.cat([-xt[..., d // 2:], xt[..., : d // 2]], -1)
+    assert np.abs((xt * cos + rot * sin).numpy() - y).max() < 1e-13
+
+
+def test_kv_proj_grad_split_equals_full_sequence_replays():
+    """dW_K = X1^T dK1 + sum_i X2(i)^T dK2(i) with the Phase-C dK1 (which already holds
+    every gK1(i)) equals the baseline's sum over the N full-sequence replays of [X1; X2(i)]^T dK(i)."""
+    inp = I.make_group(I.small_case(4, 2, 8, 11, (5, 7, 3), seed=21, dist="unit"))
+    ref = oracle.group_reference(inp)
+    rng = np.random.default_rng(3)
+    dm, N = 6, 3
+    X1 = rng.standard_normal((11, dm))
+    X2 = [rng.standard_normal((L, dm)) for L in (5, 7, 3)]
+    split = oracle.kv_proj_grad(X1, ref.dK1, X2, ref.dK2)
+    full = np.zeros_like(split)
+    for i in range(N):
+        q, k, v, dO = oracle.reference.concat_replay(inp, i, 1.0 / N)
+        r = oracle.fullseq(q, k, v, dO)
+        full += np.concatenate([X1, X2[i]]).T @ r["dk"].reshape(11 + X2[i].shape[0], -1)
+    assert np.abs(split - full).max() < 1e-10 * max(1.0, np.abs(full).max())
+    # closed form: one token, one head: dW = outer(x, dk)
+    one = oracle.kv_proj_grad(np.array([[2.0, 3.0]]), np.array([[[1.0, -1.0]]]), [], [])
+    assert np.array_equal(one, np.array([[2.0, -2.0], [3.0, -3.0]]))
