@@ -189,6 +189,33 @@ pf_status pf_segment_bwd(pf_group* grp, int64_t Ls, pf_tensor Q, pf_tensor K, pf
 /* Close the group (host-side; frees the handle only; enqueued work keeps running). */
 pf_status pf_group_end(pf_group* grp);
 
+/* Companion 1 -- rotary position embedding with positions that CONTINUE after the prefix
+ * ("Position IDs must match the baseline sequence [P||S(i)]; in particular, RoPE
+ * positions for suffix tokens continue after the prefix length rather than restarting from zero").
+ * X is a packed bf16 tensor [total, n_heads, head_dim] (pf_tensor strides), rotated IN PLACE:
+ * row r of sequence s (cu_seqlens_host[s] <= r < cu_seqlens_host[s+1]) has position
+ * pos0 + (r - cu_seqlens_host[s]) -- pos0 = 0 for the prefix, pos0 = Lp for a wave of suffixes.
+ * Rotate-half convention, theta_j = theta_base^(-2j/d), a = position * theta_j (angle formed in
+ * fp64, reduced mod 2 pi, then fp32 sin/cos):
+ *     y[j] = x[j] cos a - x[j+d/2] sin a,   y[j+d/2] = x[j+d/2] cos a + x[j] sin a,   j < d/2,
+ * computed in fp32 and rounded once to bf16.  inverse != 0 applies the transpose rotation
+ * (a -> -a): the backward of the map, to be applied to dQ / dK.  head_dim even, <= 256, multiple
+ * of 16; n_seqs >= 0 (longer tables are cut into launches of 32 sequences). */
+pf_status pf_rope(pf_ctx* ctx, int32_t n_seqs, const int32_t* cu_seqlens_host, int64_t pos0,
+                  pf_tensor X, int32_t n_heads, int32_t head_dim, float theta_base, int32_t inverse,
+                  void* stream);
+
+/* Companion 2 -- the K/V-projection weight gradient keeps the baseline's prefix-plus-suffix split
+ * (PAPER.md:212): dW_K = X1^T dK1 + sum_i X2(i)^T dK2(i); Phase B accumulates the suffix terms,
+ * Phase C adds the prefix term once from a dK1 that already contains every gK1(i).  One call adds
+ * one term:  dW[d_model, n_cols] (fp32, row-major, contiguous) += X[L, d_model]^T dY[L, n_cols]
+ * with X, dY bf16 row-major (row strides ldx, ldy in elements; dY = dK or dV viewed as
+ * [L, Hkv*d]).  A hand-written sm_100a kernel (tcgen05, fp32 accumulation in TMEM, TMA-staged
+ * tiles, split over L with a reduce-add into dW); L = 0 is a no-op. d_model and n_cols multiples
+ * of 128; X, dY 16-byte aligned, ldx, ldy multiples of 8; dW 16-byte aligned. */
+pf_status pf_kv_proj_grad(pf_ctx* ctx, int64_t L, int32_t d_model, int32_t n_cols, const void* X,
+                          int64_t ldx, const void* dY, int64_t ldy, float* dW, void* stream);
+
 /* Optional memory lifecycle: move a dormant prefix tensor (contiguous bytes)
  * to / from PINNED host memory on a side stream while Phase B runs.  Plain async copies; the
  * caller orders them against compute with events. */

@@ -25,7 +25,7 @@ SYMBOLS = ("pf_version", "pf_create", "pf_destroy", "pf_last_error", "pf_set_opt
            "pf_workspace_bytes", "pf_group_begin", "pf_phaseA_fwd", "pf_phaseB_fwd",
            "pf_phaseB_bwd", "pf_phaseC_bwd", "pf_group_end", "pf_offload", "pf_prefetch",
            "pf_counter", "pf_profile_read", "pf_group_mark_cached", "pf_segment_bwd",
-           "pf_group_set_prefix_ranges")
+           "pf_group_set_prefix_ranges", "pf_rope", "pf_kv_proj_grad")
 
 
 class PrefixFlowError(RuntimeError):
@@ -95,6 +95,10 @@ def lib() -> ctypes.CDLL:
     L.pf_group_set_prefix_ranges.argtypes = [vp, i32, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64)]
     L.pf_segment_bwd.restype = i32
     L.pf_segment_bwd.argtypes = [vp, i64, T, T, T, T, vp, T, T, vp, vp, T, T, vp]
+    L.pf_rope.restype = i32
+    L.pf_rope.argtypes = [vp, i32, pi32, i64, T, i32, i32, ctypes.c_float, i32, vp]
+    L.pf_kv_proj_grad.restype = i32
+    L.pf_kv_proj_grad.argtypes = [vp, i64, i32, i32, vp, i64, vp, i64, vp, vp]
     L.pf_offload.restype = i32
     L.pf_offload.argtypes = [vp, vp, vp, ctypes.c_size_t, vp]
     L.pf_prefetch.restype = i32
@@ -288,6 +292,32 @@ def pf_segment_bwd(grp: _Handle, Q, K, V, O, LSE, dO, dQ, accK, accV, dK, dV, st
 def pf_group_end(grp: _Handle) -> None:
     _check(lib().pf_group_end(grp.ptr), grp.ctx)
     grp.ptr = None
+
+
+def pf_rope(ctx: _Handle, cu_seqlens_host: Sequence[int], pos0: int, X: torch.Tensor, theta_base: float = 10000.0,
+            inverse: bool = False, stream=None) -> None:
+    """In-place RoPE of a packed bf16 [total, H, d] tensor; row r of sequence s sits at position
+    pos0 + (r - cu[s]) (suffix positions continue after the prefix)."""
+    _check(lib().pf_rope(ctx.ptr, len(cu_seqlens_host) - 1, _cu(cu_seqlens_host), int(pos0), as_tensor(X), int(X.shape[1]), int(X.shape[2]),
+                         float(theta_base), int(bool(inverse)), _stream(stream)), ctx)
+
+
+def pf_kv_proj_grad(ctx: _Handle, X: torch.Tensor, dY: torch.Tensor, dW: torch.Tensor, stream=None) -> None:
+    """dW[d_model, n_cols] (fp32, contiguous) += X[L, d_model]^T dY[L, n_cols]; dY may be a
+    [L, Hkv, d] tensor with contiguous (head, d) (one term of dW_K / dW_V)."""
+    if dY.dim() == 3:
+        if dY.stride(1) != dY.shape[2] or dY.stride(2) != 1:
+            raise PrefixFlowError(PF_INVALID_ARG, "pf_kv_proj_grad: dY [L, H, d] must have contiguous (H, d)")
+        n_cols, ldy = dY.shape[1] * dY.shape[2], dY.stride(0)
+    else:
+        n_cols, ldy = dY.shape[1], dY.stride(0)
+    if (X.dim() != 2 or X.dtype != torch.bfloat16 or dY.dtype != torch.bfloat16 or X.stride(1) != 1 or
+            X.shape[0] != dY.shape[0] or not X.is_cuda or not dY.is_cuda):
+        raise PrefixFlowError(PF_INVALID_ARG, "pf_kv_proj_grad: X must be a bf16 CUDA [L, d_model] matrix with as many rows as dY")
+    if (dW.dtype != torch.float32 or tuple(dW.shape) != (X.shape[1], n_cols) or not dW.is_contiguous() or not dW.is_cuda):
+        raise PrefixFlowError(PF_INVALID_ARG, f"pf_kv_proj_grad: dW must be a contiguous fp32 CUDA [{X.shape[1]}, {n_cols}] matrix")
+    _check(lib().pf_kv_proj_grad(ctx.ptr, int(X.shape[0]), int(X.shape[1]), int(n_cols), _ptr(X), int(X.stride(0)),
+                                 _ptr(dY), int(ldy), _ptr(dW), _stream(stream)), ctx)
 
 
 def pf_offload(ctx: _Handle, src_dev: torch.Tensor, dst_pinned_host: torch.Tensor, stream) -> None:

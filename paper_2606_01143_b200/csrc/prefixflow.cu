@@ -14,6 +14,7 @@
 #include "attn_fwd.cuh"
 #include "attn_bwd.cuh"
 #include "aux_kernels.cuh"
+#include "companions.cuh"
 
 namespace {
 
@@ -513,7 +514,9 @@ pf_status pf_create(pf_ctx** out, int32_t device) {
         return PF_CUDA_ERROR;
     }
     ctx->encode = reinterpret_cast<EncodeTiledFn>(fn);
-    if (set_attrs<64>() != PF_OK || set_attrs<128>() != PF_OK) {
+    if (set_attrs<64>() != PF_OK || set_attrs<128>() != PF_OK ||
+        cudaFuncSetAttribute(pf::kv_proj_grad_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             pf::GemmCfg::SMEM) != cudaSuccess) {
         delete ctx;
         return PF_CUDA_ERROR;
     }
@@ -927,6 +930,95 @@ pf_status pf_phaseC_bwd(pf_group* grp, pf_tensor Q1, pf_tensor O1, const float* 
         if (st) return st;
     }
     grp->state = 2;
+    return PF_OK;
+}
+
+pf_status pf_rope(pf_ctx* ctx, int32_t n_seqs, const int32_t* cu_seqlens_host, int64_t pos0,
+                  pf_tensor X, int32_t n_heads, int32_t head_dim, float theta_base, int32_t inverse,
+                  void* stream) {
+    if (!ctx) return PF_INVALID_ARG;
+    pf_status st;
+    if ((st = check_device(ctx))) return st;
+    if ((st = check_cu(ctx, n_seqs, cu_seqlens_host))) return st;
+    if (n_heads <= 0 || n_heads > 65535) return fail(ctx, PF_INVALID_ARG, "pf_rope: n_heads=%d", n_heads);
+    if (head_dim < 16 || head_dim > 2 * pf::kRopeMaxHalf || head_dim % 16 != 0)
+        return fail(ctx, PF_UNSUPPORTED, "pf_rope: head_dim=%d must be a multiple of 16 in [16, %d]", head_dim,
+                    2 * pf::kRopeMaxHalf);
+    if (pos0 < 0 || pos0 > (int64_t(1) << 40)) return fail(ctx, PF_INVALID_ARG, "pf_rope: pos0 out of range");
+    if (!(theta_base > 1.f) || std::isinf(theta_base))
+        return fail(ctx, PF_INVALID_ARG, "pf_rope: theta_base must be finite and > 1");
+    const int64_t total = cu_seqlens_host[n_seqs];
+    if ((st = check_tensor(ctx, "X", X, total, n_heads, head_dim))) return st;
+    if (total == 0) return PF_OK;
+    pf::RopeFreq fr;
+    memset(&fr, 0, sizeof(fr));
+    for (int j = 0; j < head_dim / 2; ++j) fr.inv[j] = std::pow(double(theta_base), -2.0 * j / head_dim);
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    int i = 0;
+    while (i < n_seqs) {   // launches of <= kMaxSeqs non-empty sequences
+        int64_t cu[pf::kMaxSeqs + 1];
+        int n = 0;
+        int64_t t0 = 0;
+        for (; i < n_seqs && n < pf::kMaxSeqs; ++i) {
+            const int64_t b = cu_seqlens_host[i], Ls = cu_seqlens_host[i + 1] - b;
+            if (Ls == 0) continue;
+            if (n == 0) { t0 = b; cu[0] = 0; }
+            cu[++n] = b + Ls - t0;
+        }
+        if (n == 0) break;
+        const pf_tensor x = tok_offset(X, t0);
+        pf::rope_kernel<<<unsigned(cu[n]), 128, 0, s>>>(static_cast<__nv_bfloat16*>(x.ptr), x.stride_tok,
+                                                        x.stride_head, n_heads, head_dim, pos0, inverse != 0,
+                                                        make_seq_table(n, cu), fr);
+        PF_CUDA(ctx, cudaGetLastError());
+        ctx->n_launches += 1;
+    }
+    return PF_OK;
+}
+
+pf_status pf_kv_proj_grad(pf_ctx* ctx, int64_t L, int32_t d_model, int32_t n_cols, const void* X,
+                          int64_t ldx, const void* dY, int64_t ldy, float* dW, void* stream) {
+    if (!ctx) return PF_INVALID_ARG;
+    pf_status st;
+    if ((st = check_device(ctx))) return st;
+    if (L < 0 || L > (int64_t(1) << 30)) return fail(ctx, PF_INVALID_ARG, "pf_kv_proj_grad: L out of range");
+    if (d_model <= 0 || n_cols <= 0 || d_model % 128 != 0 || n_cols % 128 != 0)
+        return fail(ctx, PF_UNSUPPORTED, "pf_kv_proj_grad: d_model=%d and n_cols=%d must be positive multiples of 128",
+                    d_model, n_cols);
+    if (L == 0) return PF_OK;
+    if (!X || !dY || !dW) return fail(ctx, PF_INVALID_ARG, "pf_kv_proj_grad: NULL pointer");
+    if (reinterpret_cast<uintptr_t>(X) % 16 || reinterpret_cast<uintptr_t>(dY) % 16 || reinterpret_cast<uintptr_t>(dW) % 16)
+        return fail(ctx, PF_INVALID_ARG, "pf_kv_proj_grad: X, dY and dW must be 16-byte aligned");
+    if (ldx < d_model || ldy < n_cols || ldx % 8 != 0 || ldy % 8 != 0)
+        return fail(ctx, PF_INVALID_ARG, "pf_kv_proj_grad: ldx=%lld / ldy=%lld must be >= the row length and multiples of 8",
+                    (long long)ldx, (long long)ldy);
+    CUtensorMap mX, mY;
+    const void* ptr[2] = {X, dY};
+    const int64_t ld[2] = {ldx, ldy};
+    const int cols[2] = {d_model, n_cols};
+    CUtensorMap* maps[2] = {&mX, &mY};
+    for (int i = 0; i < 2; ++i) {   // 2-D map {features, tokens}, box {64, 64}, swizzle-128B; tokens past L read as 0
+        cuuint64_t dims[2] = {cuuint64_t(cols[i]), cuuint64_t(L)};
+        cuuint64_t strides[1] = {cuuint64_t(ld[i]) * 2};
+        cuuint32_t box[2] = {64, 64};
+        cuuint32_t es[2] = {1, 1};
+        CUresult r = ctx->encode(maps[i], CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(ptr[i]), dims, strides,
+                                 box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                 CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS)
+            return fail(ctx, PF_CUDA_ERROR, "cuTensorMapEncodeTiled(%s) failed with CUresult %d", i ? "dY" : "X", int(r));
+    }
+    const int tiles = (d_model / 128) * (n_cols / 128);
+    const int n_chunks = int((L + 63) / 64);
+    int splits = (2 * ctx->num_sms + tiles - 1) / tiles;          // about two CTAs' worth of tiles per SM
+    splits = splits < 1 ? 1 : (splits > n_chunks ? n_chunks : splits);
+    const int cps = (n_chunks + splits - 1) / splits;
+    splits = (n_chunks + cps - 1) / cps;                           // no empty split
+    dim3 grid(d_model / 128, n_cols / 128, splits);
+    pf::kv_proj_grad_kernel<<<grid, pf::GemmCfg::THREADS, pf::GemmCfg::SMEM, static_cast<cudaStream_t>(stream)>>>(
+        mX, mY, dW, n_cols, n_chunks, cps);
+    PF_CUDA(ctx, cudaGetLastError());
+    ctx->n_launches += 1;
     return PF_OK;
 }
 
