@@ -372,6 +372,7 @@ def main() -> None:
                     help="suffixes packed per Phase-B call (PAPER.md:158, 242 suffix microbatch); "
                          "0 = all N in one wave (default), 1 = one call per suffix")
     ap.add_argument("--no-wave1", action="store_true", help="skip the extra wave = 1 measurement")
+    ap.add_argument("--no-companions", action="store_true", help="skip the pf_rope / pf_kv_proj_grad timings")
     ap.add_argument("--no-graph", action="store_true", help="skip the CUDA-graph replay of the step")
     ap.add_argument("--no-offload", action="store_true", help="skip the memory-lifecycle / offload measurement")
     ap.add_argument("--offload-wave", type=int, default=1, help="suffixes per wave in the lifecycle measurement")
@@ -582,6 +583,36 @@ def main() -> None:
             del gr1, g1
         torch.cuda.empty_cache()
 
+    # ---- companions: RoPE of one wave's Q2 and K2 (HBM-bound) and the
+    # dW_K terms of the step with a 7B-shaped d_model ----
+    companions = None
+    if not args.no_companions:
+        pk = g.packed[0]
+        q2, k2 = pk["Q2"].clone(), pk["K2"].clone()
+        def rope_both():
+            pf.pf_rope(ctx, pk["cu"], shape.Lp, q2, 10000.0, False, stream)
+            pf.pf_rope(ctx, pk["cu"], shape.Lp, k2, 10000.0, False, stream)
+        rope_both()
+        ms_rope = timed(rope_both, args.steps)
+        rope_bytes = 2 * (q2.numel() + k2.numel()) * 2
+        dm = 128 * shape.n_q_heads
+        X1 = torch.randn((shape.Lp, dm), device=dev).to(torch.bfloat16)
+        X2 = torch.randn((pk["K2"].shape[0], dm), device=dev).to(torch.bfloat16)
+        dW = torch.zeros((dm, shape.n_kv_heads * shape.head_dim), dtype=torch.float32, device=dev)
+        def dwk():
+            pf.pf_kv_proj_grad(ctx, X2, pk["dK2"], dW, stream)
+            pf.pf_kv_proj_grad(ctx, X1, g.dK1, dW, stream)
+        dwk()
+        ms_dw = timed(dwk, args.steps)
+        fl_dw = 2.0 * (shape.Lp + X2.shape[0]) * dm * dW.shape[1]
+        companions = dict(
+            rope=dict(ms=ms_rope, bytes=rope_bytes, gbs=rope_bytes / (ms_rope * 1e-3) / 1e9,
+                      frac_of_hbm_peak=rope_bytes / (ms_rope * 1e-3) / 1e9 / peaks["hbm"],
+                      what=f"pf_rope in place on Q2 {tuple(q2.shape)} and K2 {tuple(k2.shape)} of the wave, positions from Lp"),
+            kv_proj_grad=dict(ms=ms_dw, tflops=fl_dw / (ms_dw * 1e-3) / 1e12, flops=fl_dw,
+                              what=f"dW_K [{dm}, {dW.shape[1]}] += X2^T dK2 ({X2.shape[0]} tokens) + X1^T dK1 ({shape.Lp} tokens)"))
+        del q2, k2, X1, X2, dW
+
     # ---- memory lifecycle: Phase-B peak HBM with the dormant Phase-A set
     # {Q1, O1, LSE1} resident vs offloaded to a pinned host pool on a side stream ----
     memory = None
@@ -702,7 +733,7 @@ def main() -> None:
         metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
         ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="bf16",
         data="synthetic", config=cfg, clocks=clk.summary(), e2e=e2e, gpu_launches=launches,
-        roofline=roofline, roofline_fwd=roofline_fwd, cpu_baseline=cpu, sweep=sweep, graph=graph,
+        roofline=roofline, roofline_fwd=roofline_fwd, cpu_baseline=cpu, sweep=sweep, graph=graph, companions=companions,
         phases=phases, phaseB=dict(ms=b_ms, tflops=phaseB_tflops,
                                    pct_of_bf16_burst=100 * phaseB_tflops / peaks["burst"] if phaseB_tflops else None,
                                    pct_of_bf16_sustained=100 * phaseB_tflops / peaks["sustained"] if phaseB_tflops else None,
