@@ -244,7 +244,9 @@ def memory_legs(ctx, lifecycle, shape, dev, wave: int, layers: int, reps: int = 
     of HBM) and offloaded without any wait ("overlap").  Inputs are drawn on the device as the
     schedule asks for them (lifecycle.RandomSource): the times hold no host upload."""
     import torch
+    torch.cuda.empty_cache()
     out = dict(wave=wave, dormant_bytes_per_layer=lifecycle.dormant_bytes(shape),
+               other_live_bytes_at_start=int(torch.cuda.memory_allocated(dev)),   # counted in every peak below
                note="tensors allocated and freed as a trainer would (suffix-wave tensors live only during their "
                     "wave); peaks are torch.cuda.max_memory_allocated; pinned pool = 1.5x the dormant footprint")
     for L in ([1] + ([layers] if layers > 1 else [])):
@@ -611,7 +613,8 @@ def main() -> None:
                       what=f"pf_rope in place on Q2 {tuple(q2.shape)} and K2 {tuple(k2.shape)} of the wave, positions from Lp"),
             kv_proj_grad=dict(ms=ms_dw, tflops=fl_dw / (ms_dw * 1e-3) / 1e12, flops=fl_dw,
                               what=f"dW_K [{dm}, {dW.shape[1]}] += X2^T dK2 ({X2.shape[0]} tokens) + X1^T dK1 ({shape.Lp} tokens)"))
-        del q2, k2, X1, X2, dW
+        del q2, k2, X1, X2, dW, rope_both, dwk, pk     # the closures hold the tensors: drop them too
+        torch.cuda.empty_cache()
 
     # ---- memory lifecycle: Phase-B peak HBM with the dormant Phase-A set
     # {Q1, O1, LSE1} resident vs offloaded to a pinned host pool on a side stream ----
