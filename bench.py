@@ -561,7 +561,18 @@ def main() -> None:
                      phaseB_tflops=tf(F["B_fwd"] + F["B_bwd"], bf_ms + bb_ms),
                      phaseB_pct_of_bf16_burst=100 * tf(F["B_fwd"] + F["B_bwd"], bf_ms + bb_ms) / peaks["burst"],
                      speedup_vs_replay=(replay["ms_per_step"] / ms1) if replay else None)
-        del g1
+        # the rejected gK/gV organisation, measured next to the shipped one: every
+        # suffix adds into a partial accumulator of its own, one reduce pass before Phase C
+        pK = torch.empty((shape.N, shape.Lp, shape.n_kv_heads, shape.head_dim), dtype=torch.float32, device=dev)
+        pV = torch.empty_like(pK)
+        stepp = lambda: schedule.run_prefixflow_step_partials(ctx, g1, pK, pV, stream)
+        for _ in range(args.warmup):
+            stepp()
+        msp = timed(stepp, args.steps)
+        wave1["gkv_partials"] = dict(ms_per_step=msp, vs_reduce_add=msp / ms1,
+                                     partial_bytes=int(2 * pK.numel() * 4),
+                                     note="per-suffix fp32 partials + torch.sum reduce before Phase C (rejected alternative)")
+        del g1, pK, pV, stepp
         torch.cuda.empty_cache()
 
     # ---- the same step replayed from a CUDA graph (one launch per step: no gaps between the

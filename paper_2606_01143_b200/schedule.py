@@ -119,6 +119,42 @@ def run_prefixflow_step(ctx, g: DeviceGroup, stream=None, after_each_suffix=None
         pf.pf_group_end(grp)
 
 
+def run_prefixflow_step_partials(ctx, g: DeviceGroup, partial_K: torch.Tensor, partial_V: torch.Tensor,
+                                 stream=None) -> None:
+    """The REJECTED alternative of BASELINE.json north_star item (2), kept only so that it can be
+    measured next to the shipped accumulation: every Phase-B wave adds its prefix
+    gradients into a partial accumulator of its own (`partial_K/V` fp32 [n_waves, Lp, Hkv, d], zeroed
+    by the wave's pf_group_begin), and a reduce pass sums the partials into gK1/gV1 before Phase C.
+    The reduce is a plain elementwise torch.sum: an HBM-bound pass over n_waves x 2 x Lp x Hkv x d x 4 B."""
+    main = pf.pf_group_begin(ctx, g.desc, g.Lp, g.K1, g.V1, g.gK1, g.gV1, g.workspace, stream)
+    try:
+        pf.pf_phaseA_fwd(main, g.Q1, g.O1, g.LSE1, stream)
+        for i, pk in enumerate(g.packed):
+            grp = pf.pf_group_begin(ctx, g.desc, g.Lp, g.K1, g.V1, partial_K[i], partial_V[i], g.workspace, stream)
+            try:
+                pf.pf_group_mark_cached(grp)
+                cu = pk["cu"]
+                pf.pf_phaseB_fwd(grp, cu, pk["Q2"], pk["K2"], pk["V2"], pk["O2"], pk["LSE2"], stream)
+                pf.pf_phaseB_bwd(grp, cu, pk["Q2"], pk["K2"], pk["V2"], pk["O2"], pk["LSE2"], pk["dO2"],
+                                 pk["dQ2"], pk["dK2"], pk["dV2"], stream)
+            finally:
+                pf.pf_group_end(grp)
+        with torch.cuda.stream(stream) if isinstance(stream, torch.cuda.Stream) else _nullctx():
+            torch.sum(partial_K[:len(g.packed)], 0, out=g.gK1)
+            torch.sum(partial_V[:len(g.packed)], 0, out=g.gV1)
+        pf.pf_phaseC_bwd(main, g.Q1, g.O1, g.LSE1, g.dO1, g.dQ1, g.dK1, g.dV1, stream)
+    finally:
+        pf.pf_group_end(main)
+
+
+class _nullctx:
+    def __enter__(self):
+        return None
+
+    def __exit__(self, *a):
+        return False
+
+
 def capture_step(ctx, g: DeviceGroup, order: Optional[Sequence[int]] = None) -> "torch.cuda.CUDAGraph":
     """One A -> B -> C step captured into a CUDA graph.  Every C-ABI call only enqueues memsets and
     kernels on the caller's stream (tensor maps and kernel parameters are baked in at capture), so a

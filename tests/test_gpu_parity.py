@@ -263,6 +263,23 @@ def test_cuda_graph_replay_matches_oracle(ctx, wave):
         compare_group(g, ref)
 
 
+def test_per_wave_partials_variant_matches_oracle(ctx):
+    """The rejected gK/gV organisation (per-wave partials + a reduce pass) is a
+    different order of the same fp32 sums: same oracle, same gates."""
+    shape = inputs.small_case(4, 2, 128, 300, [129, 64, 200], seed=29, dist="unit")
+    inp = inputs.make_group(shape)
+    ref = oracle.group_reference(inp)
+    g = schedule.to_device(inp, wave=1)
+    pK = torch.full((shape.N, shape.Lp, shape.n_kv_heads, shape.head_dim), float("nan"), device="cuda")
+    pV = torch.full_like(pK, float("nan"))
+    schedule.run_prefixflow_step_partials(ctx, g, pK, pV)
+    torch.cuda.synchronize()
+    compare_group(g, ref)
+    for i in range(shape.N):
+        check(f"partial gK1[{i}]", pK[i], ref.gK1_each[i])
+        check(f"partial gV1[{i}]", pV[i], ref.gV1_each[i])
+
+
 def test_two_groups_on_two_streams(ctx):
     """No hidden shared state: two groups interleaved on two streams both match."""
     shapes = [inputs.small_case(2, 1, 64, 150, [60], seed=31), inputs.small_case(4, 4, 128, 90, [140], seed=32)]
