@@ -106,8 +106,18 @@ pf_status pf_set_option(pf_ctx* ctx, const char* name, int64_t value);
  *   "fwd_rescale_rows" : process-wide count of (query row, KV tile) events in which the forward kernel
  *                        re-based the running softmax maximum after the row's first tile (the lazy
  *                        rescale of the O accumulator).  Debug evidence for the tests; reading it
- *                        synchronises the device. */
+ *                        synchronises the device.
+ *   "last_bwd_pairs_per_item", "last_bwd_heads_per_item" : the item split the most recent backward
+ *                        launch used ((sequence, query head) pairs per prefix-tile CTA, query heads
+ *                        per causal-tile CTA): the options of the same names if set, else the split
+ *                        with the shortest simulated list-scheduling makespan over the SMs. */
 int64_t pf_counter(const pf_ctx* ctx, const char* name);
+
+/* Host-only: the backward item split the model picks for a launch of n_seqs packed sequences
+ * (cu_seqlens_host) against a prefix of Lp fully visible keys on a GPU with n_sms SMs -- what
+ * "last_bwd_*_per_item" would report after that launch with no option set.  No CUDA call is made. */
+pf_status pf_bwd_split_model(const pf_desc* desc, int64_t Lp, int32_t n_seqs, const int32_t* cu_seqlens_host,
+                             int32_t n_sms, int32_t* pairs_per_item, int32_t* heads_per_item);
 
 /* Profiling read-out (needs option "profile" = 1).  kind: the call that launched the attention
  * kernel -- 0 = pf_phaseA_fwd, 1 = pf_phaseB_fwd, 2 = pf_phaseB_bwd, 3 = pf_phaseC_bwd (forward

@@ -25,7 +25,7 @@ SYMBOLS = ("pf_version", "pf_create", "pf_destroy", "pf_last_error", "pf_set_opt
            "pf_workspace_bytes", "pf_group_begin", "pf_phaseA_fwd", "pf_phaseB_fwd",
            "pf_phaseB_bwd", "pf_phaseC_bwd", "pf_group_end", "pf_offload", "pf_prefetch",
            "pf_counter", "pf_profile_read", "pf_group_mark_cached", "pf_segment_bwd",
-           "pf_group_set_prefix_ranges", "pf_rope", "pf_kv_proj_grad")
+           "pf_group_set_prefix_ranges", "pf_rope", "pf_kv_proj_grad", "pf_bwd_split_model")
 
 
 class PrefixFlowError(RuntimeError):
@@ -95,6 +95,8 @@ def lib() -> ctypes.CDLL:
     L.pf_group_set_prefix_ranges.argtypes = [vp, i32, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64)]
     L.pf_segment_bwd.restype = i32
     L.pf_segment_bwd.argtypes = [vp, i64, T, T, T, T, vp, T, T, vp, vp, T, T, vp]
+    L.pf_bwd_split_model.restype = i32
+    L.pf_bwd_split_model.argtypes = [ctypes.POINTER(pf_desc), i64, i32, pi32, i32, pi32, pi32]
     L.pf_rope.restype = i32
     L.pf_rope.argtypes = [vp, i32, pi32, i64, T, i32, i32, ctypes.c_float, i32, vp]
     L.pf_kv_proj_grad.restype = i32
@@ -292,6 +294,16 @@ def pf_segment_bwd(grp: _Handle, Q, K, V, O, LSE, dO, dQ, accK, accV, dK, dV, st
 def pf_group_end(grp: _Handle) -> None:
     _check(lib().pf_group_end(grp.ptr), grp.ctx)
     grp.ptr = None
+
+
+def pf_bwd_split_model(desc: pf_desc, Lp: int, cu_seqlens_host: Sequence[int], n_sms: int = 148):
+    """(pairs per prefix-tile item, heads per causal-tile item) the backward would use; host-only."""
+    a, b = ctypes.c_int32(0), ctypes.c_int32(0)
+    st = lib().pf_bwd_split_model(ctypes.byref(desc), int(Lp), len(cu_seqlens_host) - 1, _cu(cu_seqlens_host),
+                                  int(n_sms), ctypes.byref(a), ctypes.byref(b))
+    if st != PF_OK:
+        raise PrefixFlowError(st, "pf_bwd_split_model: invalid arguments")
+    return a.value, b.value
 
 
 def pf_rope(ctx: _Handle, cu_seqlens_host: Sequence[int], pos0: int, X: torch.Tensor, theta_base: float = 10000.0,

@@ -5,9 +5,13 @@
 #include <cuda_runtime.h>
 #include <cstdarg>
 #include <cstdio>
+#include <cstddef>
 #include <cstring>
 #include <cmath>
+#include <algorithm>
+#include <functional>
 #include <new>
+#include <queue>
 #include <vector>
 
 #include "../../include/prefixflow.h"
@@ -34,6 +38,13 @@ struct ProfRec {
     int kind;
 };
 
+// key / value of the backward item-split model (choose_split below)
+struct SplitEntry {
+    int n, nPT, Hkv, G;
+    int cu[pf::kMaxSeqs + 1];
+    int ppcP, ppcC;
+};
+
 struct pf_ctx {
     int device = 0;
     int num_sms = 0;
@@ -44,6 +55,8 @@ struct pf_ctx {
     bool zero_accumulators = true;
     bool deterministic_gkv = false;  // one CTA per key tile: gK1/gV1/dK/dV sums in a fixed order
     int64_t n_launches = 0;
+    int last_ppcP = 0, last_ppcC = 0;      // split of the most recent backward launch (pf_counter)
+    std::vector<SplitEntry> split_cache;   // backward item splits already modelled (pf_ctx is not thread-safe)
     std::vector<ProfRec> prof;         // recorded, not yet read
     std::vector<cudaEvent_t> ev_pool;  // recycled events
     char err[512] = {0};
@@ -280,6 +293,85 @@ pf::SeqTable make_seq_table(int n, const int64_t* cu) {
     return t;
 }
 
+// ---- backward item split.  The backward launches one CTA per ITEM = (key tile, KV head, chunk of
+// the (sequence, query head) pairs that see the tile); the hardware hands items to SMs in launch
+// order as SMs free up (list scheduling).  Too few chunks leave SMs idle in the last round, too many
+// re-load K/V, re-allocate TMEM and add more partial dK/dV tiles.  Instead of a closed-form guess the
+// host SIMULATES that list scheduling for a handful of chunk sizes (cost of an item = its
+// iterations + c0 for prologue and epilogue, in units of one 128 x 64 iteration) and takes the split
+// with the shortest makespan.  Measured against the round-1 closed form (same GPU, alternating):
+// B bwd -2 % time at configs[1] packed, -7 % with one call per suffix, -6 % at configs[4], -3 % ragged.
+struct SplitModel {
+    const pf::SeqTable& seq;
+    int n, nPT, Hkv, G, sms;
+    static constexpr double kC0 = 6.0;
+    double makespan(int ppcP, int ppcC) const {
+        std::priority_queue<double, std::vector<double>, std::greater<double>> q;
+        for (int i = 0; i < sms; ++i) q.push(0.0);
+        double base = 0.0;                                  // added to every load (whole rounds of equal items)
+        auto add_equal = [&](int64_t count, double cost) {  // `count` items of the same cost, in launch order
+            base += cost * double(count / sms);
+            std::vector<double> tmp;
+            for (int64_t r = count % sms; r > 0; --r) { tmp.push_back(q.top() + cost); q.pop(); }
+            for (double v : tmp) q.push(v);
+        };
+        const int pairs = n * G;
+        if (nPT > 0 && pairs > 0) {
+            for (int lo = 0; lo < pairs; lo += ppcP) {      // chunk-major launch order
+                const int hi = std::min(pairs, lo + ppcP);
+                double it = 0;
+                for (int pr = lo; pr < hi; ++pr) it += seq.pqs[pr / G + 1] - seq.pqs[pr / G];
+                add_equal(int64_t(nPT) * Hkv, it + kC0);
+            }
+        }
+        for (int s = 0; s < n; ++s) {
+            const int nqs = seq.pqs[s + 1] - seq.pqs[s], nkt = seq.ckt[s + 1] - seq.ckt[s];
+            for (int kt = 0; kt < nkt; ++kt) {
+                const int rows = std::max(0, nqs - 2 * kt);
+                for (int c0 = 0; c0 < G; c0 += ppcC) {
+                    const int heads = std::min(G, c0 + ppcC) - c0;
+                    add_equal(Hkv, rows > 0 ? double(heads) * rows + kC0 : 0.5);
+                }
+            }
+        }
+        double mx = 0;
+        while (!q.empty()) { mx = q.top(); q.pop(); }
+        return mx + base;
+    }
+    void choose(int& ppcP, int& ppcC) const {
+        const int pairs = n * G;
+        auto items = [&](int a, int b) {
+            return int64_t(nPT) * Hkv * ((pairs + a - 1) / std::max(1, a)) + int64_t(seq.ckt[n]) * Hkv * ((G + b - 1) / b);
+        };
+        auto better = [&](double m, int64_t it, double bm, int64_t bit) {   // 0.5 % ties go to fewer items
+            return m < bm * 0.995 || (m <= bm * 1.005 && it < bit && m < bm * 1.005);
+        };
+        static const int kChunks[] = {1, 2, 3, 4, 5, 6, 7, 8, 10, 12, 14, 16, 20, 24, 28, 32, 40, 48, 56, 64, 96, 128};
+        for (int pass = 0; pass < 2; ++pass) {
+            if (nPT > 0 && pairs > 0) {                     // pairs per prefix item, even chunks only
+                double bm = 1e300; int64_t bit = 0; int best = ppcP, last = -1;
+                for (int ch : kChunks) {
+                    if (ch > pairs) break;
+                    const int a = (pairs + ch - 1) / ch;
+                    if (a == last) continue;
+                    last = a;
+                    const double m = makespan(a, ppcC);
+                    if (better(m, items(a, ppcC), bm, bit)) { bm = m; bit = items(a, ppcC); best = a; }
+                }
+                ppcP = best;
+            }
+            double bm = 1e300; int64_t bit = 0; int best = ppcC;
+            for (int b = 1; b <= G; ++b) {                  // query heads per causal item
+                if (b > 1 && (G + b - 1) / b == (G + b - 2) / (b - 1)) continue;   // same chunk count as b - 1
+                const double m = makespan(ppcP, b);
+                if (better(m, items(ppcP, b), bm, bit)) { bm = m; bit = items(ppcP, b); best = b; }
+            }
+            if (best == ppcC && pass > 0) break;
+            ppcC = best;
+        }
+    }
+};
+
 // ---- forward launch over n sequences packed along the token axis: the queries of sequence s
 // attend to the prefix source [Lp] (all visible) + the keys of s causally
 // `prefix`: cached maps of the prefix source (NULL when Lp = 0); `causal`: cached maps of the causal
@@ -397,29 +489,33 @@ pf_status launch_bwd(pf_group* g, const pf_tensor& Q, const KvMaps* prefix, cons
     p.nPT = p.pre.n > 0 ? p.pre.tile0[p.pre.n] : 0;
     p.nQS = nQS;
     p.seq = seq;
-    // ---- item sizing: aim at >= ~6 items per SM, each long enough to amortise its prologue
-    // (K/V load, TMEM allocation) and epilogue (dK/dV reduce-add)
-    int64_t iters = int64_t(p.nPT) * Hkv * G * nQS;
-    for (int i = 0; i < n; ++i) {
-        const int nqs = seq.pqs[i + 1] - seq.pqs[i], nkt = seq.ckt[i + 1] - seq.ckt[i];
-        for (int kt = 0; kt < nkt; ++kt) iters += int64_t(Hkv) * G * (nqs - 2 * kt > 0 ? nqs - 2 * kt : 0);
-    }
-    const double target = std::fmin(192.0, std::fmax(24.0, double(iters) / (6.0 * ctx->num_sms)));
-    const double avg_nqs = n > 0 ? double(nQS) / n : 1.0;
+    // ---- item sizing (SplitModel above); options and deterministic_gkv override the model
     const int pairs = n * G;
-    int ppcP = ctx->deterministic_gkv ? pairs
-               : ctx->bwd_pairs_per_item > 0 ? ctx->bwd_pairs_per_item
-                                             : int(std::lround(target / std::fmax(1.0, avg_nqs)));
-    ppcP = ppcP < 1 ? 1 : (ppcP > pairs ? pairs : ppcP);
-    if (ctx->bwd_pairs_per_item == 0 && !ctx->deterministic_gkv && pairs > 0) {   // even chunks: no tiny last item
-        const int chunks = (pairs + ppcP - 1) / ppcP;
-        ppcP = (pairs + chunks - 1) / chunks;
+    int ppcP = pairs > 0 ? pairs : 1, ppcC = (G + 1) / 2;
+    if (ctx->deterministic_gkv) {
+        ppcC = G;
+    } else {
+        SplitEntry key;
+        memset(&key, 0, sizeof(key));
+        key.n = n; key.nPT = p.nPT; key.Hkv = Hkv; key.G = G;
+        for (int i = 0; i <= n; ++i) key.cu[i] = seq.cu[i];
+        const SplitEntry* hit = nullptr;
+        for (const SplitEntry& e : ctx->split_cache)
+            if (memcmp(&e, &key, offsetof(SplitEntry, ppcP)) == 0) { hit = &e; break; }
+        if (!hit) {
+            key.ppcP = ppcP; key.ppcC = ppcC;
+            SplitModel{seq, n, p.nPT, Hkv, G, ctx->num_sms}.choose(key.ppcP, key.ppcC);
+            if (ctx->split_cache.size() >= 64) ctx->split_cache.erase(ctx->split_cache.begin());
+            ctx->split_cache.push_back(key);
+            hit = &ctx->split_cache.back();
+        }
+        ppcP = hit->ppcP; ppcC = hit->ppcC;
+        if (ctx->bwd_pairs_per_item > 0) ppcP = ctx->bwd_pairs_per_item;
+        if (ctx->bwd_heads_per_item > 0) ppcC = ctx->bwd_heads_per_item;
     }
-    int ppcC = ctx->deterministic_gkv ? G
-               : ctx->bwd_heads_per_item > 0 ? ctx->bwd_heads_per_item
-                                             : int(std::lround(target / std::fmax(1.0, avg_nqs)));
-    const int capC = (ctx->bwd_heads_per_item > 0 || ctx->deterministic_gkv) ? G : (G + 1) / 2;   // measured: G heads per causal item is too coarse
-    ppcC = ppcC < 1 ? 1 : (ppcC > capC ? capC : ppcC);
+    ppcP = ppcP < 1 ? 1 : (ppcP > pairs && pairs > 0 ? pairs : ppcP);
+    ppcC = ppcC < 1 ? 1 : (ppcC > G ? G : ppcC);
+    ctx->last_ppcP = ppcP; ctx->last_ppcC = ppcC;
     p.ppcP = ppcP; p.chunksP = (pairs + ppcP - 1) / ppcP;
     p.ppcC = ppcC; p.chunksC = (G + ppcC - 1) / ppcC;
     p.nItemsP = p.nPT * Hkv * p.chunksP;
@@ -562,12 +658,34 @@ pf_status pf_set_option(pf_ctx* ctx, const char* name, int64_t value) {
 int64_t pf_counter(const pf_ctx* ctx, const char* name) {
     if (!ctx || !name) return -1;
     if (strcmp(name, "kernel_launches") == 0) return ctx->n_launches;
+    if (strcmp(name, "last_bwd_pairs_per_item") == 0) return ctx->last_ppcP;
+    if (strcmp(name, "last_bwd_heads_per_item") == 0) return ctx->last_ppcC;
     if (strcmp(name, "fwd_rescale_rows") == 0) {   // device-side debug counter (synchronises)
         unsigned long long v = 0;
         if (cudaMemcpyFromSymbol(&v, pf::g_fwd_rescale_rows, sizeof(v)) != cudaSuccess) return -1;
         return int64_t(v);
     }
     return -1;
+}
+
+pf_status pf_bwd_split_model(const pf_desc* desc, int64_t Lp, int32_t n_seqs, const int32_t* cu_seqlens_host,
+                             int32_t n_sms, int32_t* pairs_per_item, int32_t* heads_per_item) {
+    if (!desc || !cu_seqlens_host || !pairs_per_item || !heads_per_item) return PF_INVALID_ARG;
+    if (desc->n_q_heads <= 0 || desc->n_kv_heads <= 0 || desc->n_q_heads % desc->n_kv_heads != 0 ||
+        n_seqs < 0 || n_seqs > pf::kMaxSeqs || n_sms <= 0 || Lp < 0 || cu_seqlens_host[0] != 0)
+        return PF_INVALID_ARG;
+    int64_t cu[pf::kMaxSeqs + 1];
+    for (int i = 0; i <= n_seqs; ++i) {
+        if (i > 0 && cu_seqlens_host[i] < cu_seqlens_host[i - 1]) return PF_INVALID_ARG;
+        cu[i] = cu_seqlens_host[i];
+    }
+    const pf::SeqTable seq = make_seq_table(n_seqs, cu);
+    const int G = desc->n_q_heads / desc->n_kv_heads;
+    int a = n_seqs * G > 0 ? n_seqs * G : 1, b = (G + 1) / 2;
+    SplitModel{seq, n_seqs, int((Lp + 127) / 128), desc->n_kv_heads, G, n_sms}.choose(a, b);
+    *pairs_per_item = a;
+    *heads_per_item = b;
+    return PF_OK;
 }
 
 pf_status pf_profile_read(pf_ctx* ctx, int32_t kind, int64_t* launches, double* total_ms) {

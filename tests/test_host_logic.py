@@ -38,3 +38,26 @@ def test_wave_partition_and_ragged_recipe():
     assert schedule._waves(3, 0) == [[0], [1], [2]] and schedule._waves(0, 4) == []
     Ls = inputs.config_ragged().Ls
     assert len(Ls) == 16 and all(256 <= x <= 2048 for x in Ls) and Ls == inputs.config_ragged().Ls
+
+
+def test_bwd_split_model_is_host_only_deterministic_and_even():
+    """The backward item split comes from a list-scheduling simulation on the host (prefixflow.cu
+    SplitModel): no GPU needed.  configs[1], one packed wave on 148 SMs: 8 x 7 = 56 pairs in 4 even
+    chunks of 14 -- the split measured fastest on the B200 (profiles/r2_kernel_experiments.md)."""
+    from paper_2606_01143_b200 import binding as pf
+    d = pf.make_desc(28, 4, 128)
+    cu8 = [1024 * i for i in range(9)]
+    a, b = pf.pf_bwd_split_model(d, 5120, cu8)
+    assert (a, b) == pf.pf_bwd_split_model(d, 5120, cu8)
+    assert a == 14 and 56 % a == 0 and 1 <= b <= 7
+    # Phase C / replay: no prefix source, one sequence: only the heads-per-item choice matters
+    a1, b1 = pf.pf_bwd_split_model(d, 0, [0, 5120])
+    assert 1 <= b1 <= 7 and a1 >= 1
+    # one call per suffix: fewer pairs per item than the packed wave (more parallelism is needed)
+    a2, _ = pf.pf_bwd_split_model(d, 5120, [0, 1024])
+    assert 1 <= a2 < a
+    # a tiny launch on a big GPU is split as finely as it can be; a one-SM GPU gets whole key tiles
+    assert pf.pf_bwd_split_model(pf.make_desc(2, 2, 64), 256, [0, 64], 148)[0] == 1
+    assert pf.pf_bwd_split_model(d, 5120, cu8, 1) == (56, 7)
+    with __import__("pytest").raises(pf.PrefixFlowError):
+        pf.pf_bwd_split_model(d, 5120, [0, 10, 5])
