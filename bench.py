@@ -380,6 +380,7 @@ def main() -> None:
     ap.add_argument("--offload-wave", type=int, default=1, help="suffixes per wave in the lifecycle measurement")
     ap.add_argument("--layers", type=int, default=4, help="attention layers in the multi-layer offload pipeline (0 = skip)")
     ap.add_argument("--bwd-pairs", type=int, default=0, help="C-ABI option bwd_pairs_per_item (0 = heuristic)")
+    ap.add_argument("--bwd-heads", type=int, default=0, help="C-ABI option bwd_heads_per_item (0 = model)")
     ap.add_argument("--deterministic", action="store_true", help="C-ABI option deterministic_gkv")
     ap.add_argument("--no-sweep", action="store_true", help="skip the compact prefix-ratio x N sweep / configs[2], configs[4] legs")
     ap.add_argument("--shard", default="groups", choices=["groups", "heads", "split"],
@@ -415,6 +416,8 @@ def main() -> None:
     ctx = pf.pf_create(local_rank)
     if args.bwd_pairs:
         pf.pf_set_option(ctx, "bwd_pairs_per_item", args.bwd_pairs)
+    if args.bwd_heads:
+        pf.pf_set_option(ctx, "bwd_heads_per_item", args.bwd_heads)
     if args.deterministic:
         pf.pf_set_option(ctx, "deterministic_gkv", 1)
     if world > 1 and args.shard != "groups":

@@ -299,75 +299,95 @@ pf::SeqTable make_seq_table(int n, const int64_t* cu) {
 // re-load K/V, re-allocate TMEM and add more partial dK/dV tiles.  Instead of a closed-form guess the
 // host SIMULATES that list scheduling for a handful of chunk sizes (cost of an item = its
 // iterations + c0 for prologue and epilogue, in units of one 128 x 64 iteration) and takes the split
-// with the shortest makespan.  Measured against the round-1 closed form (same GPU, alternating):
-// B bwd -2 % time at configs[1] packed, -7 % with one call per suffix, -6 % at configs[4], -3 % ragged.
+// with the shortest makespan.  Fitted on one-call-per-suffix launches of configs[1]: c0 = 6 predicts the
+// measured kernel times of 15 splits within 1.8 % on average.  Measured against the round-1 closed form
+// (fresh processes, alternating, same GPU; profiles/r2_kernel_experiments.md): configs[1] B bwd +2 %,
+// C bwd +8 %, one call per suffix +4.5 %; configs[4] C bwd +14 %, whole step -9 % time.
 struct SplitModel {
     const pf::SeqTable& seq;
     int n, nPT, Hkv, G, sms;
     static constexpr double kC0 = 6.0;
-    double makespan(int ppcP, int ppcC) const {
-        std::priority_queue<double, std::vector<double>, std::greater<double>> q;
-        for (int i = 0; i < sms; ++i) q.push(0.0);
-        double base = 0.0;                                  // added to every load (whole rounds of equal items)
-        auto add_equal = [&](int64_t count, double cost) {  // `count` items of the same cost, in launch order
-            base += cost * double(count / sms);
-            std::vector<double> tmp;
-            for (int64_t r = count % sms; r > 0; --r) { tmp.push_back(q.top() + cost); q.pop(); }
-            for (double v : tmp) q.push(v);
-        };
-        const int pairs = n * G;
-        if (nPT > 0 && pairs > 0) {
-            for (int lo = 0; lo < pairs; lo += ppcP) {      // chunk-major launch order
-                const int hi = std::min(pairs, lo + ppcP);
-                double it = 0;
-                for (int pr = lo; pr < hi; ++pr) it += seq.pqs[pr / G + 1] - seq.pqs[pr / G];
-                add_equal(int64_t(nPT) * Hkv, it + kC0);
-            }
+    // exact list scheduling in the kernel's launch order on a binary min-heap `h` of SM finish times
+    static void give(std::vector<double>& h, double cost) {  // next item goes to the SM that frees up first
+        const int sms = int(h.size());
+        const double v = h[0] + cost;
+        int i = 0;
+        for (;;) {                                          // sift down
+            int c = 2 * i + 1;
+            if (c >= sms) break;
+            if (c + 1 < sms && h[c + 1] < h[c]) ++c;
+            if (h[c] >= v) break;
+            h[i] = h[c];
+            i = c;
         }
+        h[i] = v;
+    }
+    void prefix_phase(int ppcP, std::vector<double>& h) const {
+        h.assign(sms, 0.0);
+        const int pairs = n * G;
+        if (nPT == 0 || pairs == 0) return;
+        for (int lo = 0; lo < pairs; lo += ppcP) {          // chunk-major: all key tiles of a chunk cost the same
+            const int hi = std::min(pairs, lo + ppcP);
+            double it = 0;
+            for (int pr = lo; pr < hi; ++pr) it += seq.pqs[pr / G + 1] - seq.pqs[pr / G];
+            int64_t cnt = int64_t(nPT) * Hkv;
+            const double cost = it + kC0;
+            // whole rounds of equal items give every SM one item each -- exactly what list
+            // scheduling does as long as the finish times differ by no more than one item
+            if (cnt >= sms && *std::max_element(h.begin(), h.end()) - h[0] <= cost) {
+                const double add = cost * double(cnt / sms);
+                for (double& v : h) v += add;
+                cnt %= sms;
+            }
+            for (; cnt > 0; --cnt) give(h, cost);
+        }
+    }
+    double causal_phase(int ppcC, std::vector<double>& h) const {
         for (int s = 0; s < n; ++s) {
             const int nqs = seq.pqs[s + 1] - seq.pqs[s], nkt = seq.ckt[s + 1] - seq.ckt[s];
             for (int kt = 0; kt < nkt; ++kt) {
                 const int rows = std::max(0, nqs - 2 * kt);
-                for (int c0 = 0; c0 < G; c0 += ppcC) {
-                    const int heads = std::min(G, c0 + ppcC) - c0;
-                    add_equal(Hkv, rows > 0 ? double(heads) * rows + kC0 : 0.5);
-                }
+                for (int g = 0; g < Hkv; ++g)
+                    for (int c0 = 0; c0 < G; c0 += ppcC)
+                        give(h, rows > 0 ? double(std::min(G, c0 + ppcC) - c0) * rows + kC0 : 0.5);
             }
         }
-        double mx = 0;
-        while (!q.empty()) { mx = q.top(); q.pop(); }
-        return mx + base;
+        return *std::max_element(h.begin(), h.end());
     }
     void choose(int& ppcP, int& ppcC) const {
         const int pairs = n * G;
-        auto items = [&](int a, int b) {
-            return int64_t(nPT) * Hkv * ((pairs + a - 1) / std::max(1, a)) + int64_t(seq.ckt[n]) * Hkv * ((G + b - 1) / b);
-        };
-        auto better = [&](double m, int64_t it, double bm, int64_t bit) {   // 0.5 % ties go to fewer items
-            return m < bm * 0.995 || (m <= bm * 1.005 && it < bit && m < bm * 1.005);
-        };
         static const int kChunks[] = {1, 2, 3, 4, 5, 6, 7, 8, 10, 12, 14, 16, 20, 24, 28, 32, 40, 48, 56, 64, 96, 128};
-        for (int pass = 0; pass < 2; ++pass) {
-            if (nPT > 0 && pairs > 0) {                     // pairs per prefix item, even chunks only
-                double bm = 1e300; int64_t bit = 0; int best = ppcP, last = -1;
-                for (int ch : kChunks) {
-                    if (ch > pairs) break;
-                    const int a = (pairs + ch - 1) / ch;
-                    if (a == last) continue;
-                    last = a;
-                    const double m = makespan(a, ppcC);
-                    if (better(m, items(a, ppcC), bm, bit)) { bm = m; bit = items(a, ppcC); best = a; }
+        std::vector<int> as, bs;                            // candidate pairs per prefix item / heads per causal item
+        if (nPT > 0 && pairs > 0) {
+            const double per_chunk = double(nPT) * Hkv / sms;   // prefix items per SM and chunk
+            for (int ch : kChunks) {
+                if (ch > pairs) break;
+                if (ch > 1 && ch * per_chunk > 16.0) break;     // more than ~16 prefix items per SM never paid
+                const int a = (pairs + ch - 1) / ch;
+                if (as.empty() || as.back() != a) as.push_back(a);
+            }
+        } else {
+            as.push_back(std::max(1, pairs));
+        }
+        for (int b : {1, 2, (G + 1) / 2, G})                // the most even split of 1, 2, ~G/2 and G heads per item
+            if (b >= 1 && b <= G && std::find(bs.begin(), bs.end(), b) == bs.end()) bs.push_back(b);
+        double bm = 1e300;
+        std::vector<double> after_prefix, h;
+        for (int a : as) {
+            prefix_phase(a, after_prefix);
+            for (int b : bs) {
+                h = after_prefix;
+                const double m = causal_phase(b, h);
+                if (getenv("PF_SPLIT_DEBUG")) fprintf(stderr, "split a=%d b=%d makespan=%.1f\n", a, b, m);
+                // ties (0.2 %): fewer, longer items -- less K/V re-loading, and CTAs that run side by
+                // side then walk the same query heads, which keeps their Q / dO tiles in L2 (measured at
+                // configs[4]: 2 instead of 5 heads per causal item costs Phase C 44 %)
+                const bool tie = m <= bm * 1.002 && m >= bm * 0.998;
+                const bool tie_better = a > ppcP || (a == ppcP && b > ppcC);
+                if (m < bm * 0.998 || (tie && tie_better)) {
+                    bm = std::min(bm, m); ppcP = a; ppcC = b;
                 }
-                ppcP = best;
             }
-            double bm = 1e300; int64_t bit = 0; int best = ppcC;
-            for (int b = 1; b <= G; ++b) {                  // query heads per causal item
-                if (b > 1 && (G + b - 1) / b == (G + b - 2) / (b - 1)) continue;   // same chunk count as b - 1
-                const double m = makespan(ppcP, b);
-                if (better(m, items(ppcP, b), bm, bit)) { bm = m; bit = items(ppcP, b); best = b; }
-            }
-            if (best == ppcC && pass > 0) break;
-            ppcC = best;
         }
     }
 };
