@@ -263,6 +263,35 @@ def test_cuda_graph_replay_matches_oracle(ctx, wave):
         compare_group(g, ref)
 
 
+def _random_shapes(count, seed):
+    rng = np.random.default_rng(seed)
+    out = []
+    for i in range(count):
+        d = int(rng.choice([64, 128]))
+        Hkv = int(rng.choice([1, 2, 3, 4]))
+        G = int(rng.choice([1, 2, 4, 7]))
+        Lp = int(rng.choice([0, 33, 64, 127, 128, 129, 200, 333, 512, 700]))
+        n = int(rng.integers(1, 6))
+        Ls = [int(rng.choice([0, 1, 17, 63, 64, 65, 128, 130, 191, 257, 300])) for _ in range(n)]
+        wave = int(rng.integers(1, n + 1))
+        dist = ["std", "unit", "spike"][i % 3]
+        out.append((G * Hkv, Hkv, d, Lp, Ls, wave, dist))
+    return out
+
+
+@pytest.mark.parametrize("Hq,Hkv,d,Lp,Ls,wave,dist", _random_shapes(24, 20260611))
+def test_random_shapes(ctx, Hq, Hkv, d, Lp, Ls, wave, dist):
+    """Seeded random small groups (head counts, unaligned prefix / suffix lengths incl. empty ones, wave
+    sizes, all three input distributions): every launch shape gets its own backward item split from
+    the scheduling model, so this also walks many different (pairs, heads) chunkings.  "spike" rows are
+    nearly one-hot: forward gates only, as in test_adversarial_logits; one- and two-key rows with unit
+    logits are test_smallest_nonempty's subject (derived bound), so prefixes here have >= 33 tokens."""
+    if sum(Ls) == 0 and Lp == 0:
+        pytest.skip("empty group")
+    run_and_compare(ctx, inputs.small_case(Hq, Hkv, d, Lp, Ls, seed=1000 + Lp + sum(Ls), dist=dist), wave=wave,
+                    backward=(dist != "spike"))
+
+
 def test_per_wave_partials_variant_matches_oracle(ctx):
     """The rejected gK/gV organisation (per-wave partials + a reduce pass) is a
     different order of the same fp32 sums: same oracle, same gates."""
