@@ -123,6 +123,20 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
     const int nP = p.pre.n > 0 ? p.pre.tile0[p.pre.n] : 0;
     const int n_iter = nP + rb + 1;
 
+    // The softmax threads put their loads of Q in flight BEFORE the set-up barrier (mbarrier init,
+    // TMEM allocation), so that the round trip to L2 / HBM overlaps the set-up instead of following it.
+    constexpr int QW = D / 8;                    // 32-bit words of Q per softmax thread (a quarter row)
+    uint32_t qv[QW];
+    if (warp < 16) {
+        const int r = tid & 127, qd = warp >> 2, t = rb * 128 + r;
+        const uint4* qrow = reinterpret_cast<const uint4*>(
+            p.Q + int64_t(tok0 + t) * p.q_stride_tok + int64_t(h) * p.q_stride_head + qd * (D / 4));
+#pragma unroll
+        for (int j = 0; j < QW / 4; ++j) {
+            const uint4 v = t < Ls ? __ldg(qrow + j) : make_uint4(0u, 0u, 0u, 0u);
+            qv[4 * j] = v.x; qv[4 * j + 1] = v.y; qv[4 * j + 2] = v.z; qv[4 * j + 3] = v.w;
+        }
+    }
     if (tid == 0) {
         mbar_init(bar_Q, 512);
         for (int s = 0; s < C::KS; ++s) {
@@ -229,14 +243,6 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
         const float c = p.scale_log2;
         // ---- Q row -> TMEM (A operand layout: lane = row, column j = elements 2j, 2j+1)
         {
-            const uint4* qrow = reinterpret_cast<const uint4*>(
-                p.Q + int64_t(tok0 + t) * p.q_stride_tok + int64_t(h) * p.q_stride_head + qd * DQ);
-            uint32_t qv[DQ / 2];
-#pragma unroll
-            for (int j = 0; j < DQ / 8; ++j) {
-                const uint4 v = valid ? qrow[j] : make_uint4(0u, 0u, 0u, 0u);
-                qv[4 * j] = v.x; qv[4 * j + 1] = v.y; qv[4 * j + 2] = v.z; qv[4 * j + 3] = v.w;
-            }
             if constexpr (D == 128) tmem_st16(tmem + C::T_Q + qd * 16 + lane_off, qv);
             else tmem_st8(tmem + C::T_Q + qd * 8 + lane_off, qv);
             tmem_wait_st();
