@@ -137,12 +137,27 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
             qv[4 * j] = v.x; qv[4 * j + 1] = v.y; qv[4 * j + 2] = v.z; qv[4 * j + 3] = v.w;
         }
     }
+    // one K/V tile of iteration `it` into ring stage it % KS (TMA producer thread only)
+    auto load_tile = [&](int it) {
+        const int st = it % C::KS;
+        const uint32_t ph = (it / C::KS) & 1;
+        const bool pre = it < nP;
+        int row0 = tok0 + (it - nP) * 128, valid_rows;
+        if (pre) p.pre.locate(it, row0, valid_rows);
+        mbar_wait(&bar_Ke[st], ph ^ 1);
+        mbar_arrive_expect_tx(&bar_Kf[st], C::TILE);
+        for (int k = 0; k < C::NSUB; ++k)
+            tma_load_3d(smem + C::OFF_K + st * C::TILE + k * C::SUB, pre ? &tmK1 : &tmK2,
+                        &bar_Kf[st], 64 * k, g, row0);
+        mbar_wait(&bar_Ve[st], ph ^ 1);
+        mbar_arrive_expect_tx(&bar_Vf[st], C::TILE);
+        for (int k = 0; k < C::NSUB; ++k)
+            tma_load_3d(smem + C::OFF_V + st * C::TILE + k * C::SUB, pre ? &tmV1 : &tmV2,
+                        &bar_Vf[st], 64 * k, g, row0);
+    };
+    const int n_early = n_iter < C::KS ? n_iter : C::KS;   // tiles whose loads go out before the set-up barrier
     if (tid == 0) {
         mbar_init(bar_Q, 512);
-        for (int s = 0; s < C::KS; ++s) {
-            mbar_init(&bar_Kf[s], 1); mbar_init(&bar_Ke[s], 1);
-            mbar_init(&bar_Vf[s], 1); mbar_init(&bar_Ve[s], 1);
-        }
         mbar_init(&bar_S[0], 1); mbar_init(&bar_S[1], 1);
         for (int i = 0; i < 4; ++i) mbar_init(&bar_P[i], 256);
         mbar_init(bar_PV, 1);
@@ -150,11 +165,20 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
         fence_mbar_init();
     }
     if (warp == 16) {
-        tmem_alloc(tmem_slot, 512);
+        // the producer initialises its own ring barriers and fills the ring right away: the first K/V
+        // tiles travel while TMEM is allocated and Q is on its way
         if (elect_one()) {
+            for (int s = 0; s < C::KS; ++s) {
+                mbar_init(&bar_Kf[s], 1); mbar_init(&bar_Ke[s], 1);
+                mbar_init(&bar_Vf[s], 1); mbar_init(&bar_Ve[s], 1);
+            }
+            fence_mbar_init();
             tma_prefetch_desc(&tmK1); tma_prefetch_desc(&tmV1);
             tma_prefetch_desc(&tmK2); tma_prefetch_desc(&tmV2);
+            for (int it = 0; it < n_early; ++it) load_tile(it);
         }
+        __syncwarp();
+        tmem_alloc(tmem_slot, 512);
     }
     tc_fence_before();
     __syncthreads();
@@ -164,23 +188,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
     if (warp == 16) {
         // =============================== TMA producer ===============================
         if (elect_one()) {
-            for (int it = 0; it < n_iter; ++it) {
-                const int st = it % C::KS;
-                const uint32_t ph = (it / C::KS) & 1;
-                const bool pre = it < nP;
-                int row0 = tok0 + (it - nP) * 128, valid_rows;
-                if (pre) p.pre.locate(it, row0, valid_rows);
-                mbar_wait(&bar_Ke[st], ph ^ 1);
-                mbar_arrive_expect_tx(&bar_Kf[st], C::TILE);
-                for (int k = 0; k < C::NSUB; ++k)
-                    tma_load_3d(smem + C::OFF_K + st * C::TILE + k * C::SUB, pre ? &tmK1 : &tmK2,
-                                &bar_Kf[st], 64 * k, g, row0);
-                mbar_wait(&bar_Ve[st], ph ^ 1);
-                mbar_arrive_expect_tx(&bar_Vf[st], C::TILE);
-                for (int k = 0; k < C::NSUB; ++k)
-                    tma_load_3d(smem + C::OFF_V + st * C::TILE + k * C::SUB, pre ? &tmV1 : &tmV2,
-                                &bar_Vf[st], 64 * k, g, row0);
-            }
+            for (int it = n_early; it < n_iter; ++it) load_tile(it);
         }
     } else if (warp == 17) {
         // =============================== MMA issuer ===============================
