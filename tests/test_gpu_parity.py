@@ -292,6 +292,39 @@ def test_random_shapes(ctx, Hq, Hkv, d, Lp, Ls, wave, dist):
                     backward=(dist != "spike"))
 
 
+def test_backward_uses_the_modelled_split_and_options_override_it(ctx):
+    """The counters report the item split of the last backward launch: the host model's choice
+    (pf_bwd_split_model with the device's SM count) unless an option pins it."""
+    shape = inputs.small_case(8, 2, 128, 700, [300, 129, 200], seed=41)
+    g = schedule.random_device_group(shape, "cuda", wave=3, seed=2)
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    schedule.run_prefixflow_step(ctx, g)                      # last backward launch = Phase C
+    want = pf.pf_bwd_split_model(g.desc, 0, [0, shape.Lp], sms)
+    assert pf.pf_counter(ctx, "last_bwd_heads_per_item") == want[1]
+    grp = pf.pf_group_begin(ctx, g.desc, g.Lp, g.K1, g.V1, g.gK1, g.gV1, g.workspace)
+    try:
+        pf.pf_phaseA_fwd(grp, g.Q1, g.O1, g.LSE1)
+        pk = g.packed[0]
+        pf.pf_phaseB_fwd(grp, pk["cu"], pk["Q2"], pk["K2"], pk["V2"], pk["O2"], pk["LSE2"])
+        pf.pf_phaseB_bwd(grp, pk["cu"], pk["Q2"], pk["K2"], pk["V2"], pk["O2"], pk["LSE2"], pk["dO2"],
+                         pk["dQ2"], pk["dK2"], pk["dV2"])
+        want = pf.pf_bwd_split_model(g.desc, shape.Lp, pk["cu"], sms)
+        got = (pf.pf_counter(ctx, "last_bwd_pairs_per_item"), pf.pf_counter(ctx, "last_bwd_heads_per_item"))
+        assert got == want, (got, want)
+        pf.pf_set_option(ctx, "bwd_pairs_per_item", 5)
+        pf.pf_set_option(ctx, "bwd_heads_per_item", 3)
+        try:
+            pf.pf_phaseB_bwd(grp, pk["cu"], pk["Q2"], pk["K2"], pk["V2"], pk["O2"], pk["LSE2"], pk["dO2"],
+                             pk["dQ2"], pk["dK2"], pk["dV2"])
+            assert (pf.pf_counter(ctx, "last_bwd_pairs_per_item"), pf.pf_counter(ctx, "last_bwd_heads_per_item")) == (5, 3)
+        finally:
+            pf.pf_set_option(ctx, "bwd_pairs_per_item", 0)
+            pf.pf_set_option(ctx, "bwd_heads_per_item", 0)
+    finally:
+        pf.pf_group_end(grp)
+    torch.cuda.synchronize()
+
+
 def test_per_wave_partials_variant_matches_oracle(ctx):
     """The rejected gK/gV organisation (per-wave partials + a reduce pass) is a
     different order of the same fp32 sums: same oracle, same gates."""
