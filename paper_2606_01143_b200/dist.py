@@ -277,3 +277,65 @@ def run_split_group_step(rank: SplitGroupRank, comm: DistComm, comm_stream=None)
     w3 = ev(); w3.record(main)
     rank.phase_c(rank.gK1s, rank.gV1s)
     return dict(gather_wait=(w0, w1), reduce_wait=(w2, w3))
+
+
+class SelfComm:
+    """world = 1: the collectives of `DistComm` as identities (a copy), with the same signatures.
+    Lets the stream / event schedule of the multi-layer step run on one GPU without a process group."""
+    world, rank = 1, 0
+
+    def all_gather_heads(self, shard: torch.Tensor) -> torch.Tensor:
+        return shard.clone()
+
+    def reduce_scatter_heads(self, full: torch.Tensor, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+        if out is None:
+            return full.clone()
+        out.copy_(full)
+        return out
+
+
+def run_split_group_layers(layers: Sequence[SplitGroupRank], comm, comm_stream: torch.cuda.Stream) -> dict:
+    """One rank's step over L attention layers of a split group with the exchanges overlapped
+    ("next-layer K/V gathers and previous-layer gK/gV reductions are prefetched on a
+    communication stream", :310): Phase A runs layer by layer and each layer's K1/V1 all-gather is
+    enqueued on `comm_stream` right behind it -- it travels under the Phase A of the later layers and
+    the Phase B of the earlier ones; each layer's gK1/gV1 reduce-scatter is enqueued right behind its
+    Phase B and travels under the Phase B of the later layers; Phase C runs in reverse layer order
+    and waits only for its own layer's reduction.  `layers[l]` holds the rank's tensors of layer l.
+    Returns the milliseconds the compute stream spent waiting for a gather / a reduction (exposed
+    communication) once the caller has synchronised."""
+    main = layers[0].stream if isinstance(layers[0].stream, torch.cuda.Stream) else torch.cuda.current_stream()
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    gathered, g_done, r_done, waits = [], [], [], []
+    for rk in layers:                                          # Phase A + gather behind it
+        rk.phase_a()
+        a = ev(); a.record(main)
+        comm_stream.wait_event(a)
+        with torch.cuda.stream(comm_stream):
+            gathered.append((comm.all_gather_heads(rk.K1), comm.all_gather_heads(rk.V1)))
+            e = ev(); e.record(comm_stream)
+        g_done.append(e)
+    for l, rk in enumerate(layers):                            # Phase B + reduction behind it
+        w0 = ev(); w0.record(main)
+        main.wait_event(g_done[l])
+        w1 = ev(); w1.record(main)
+        waits.append(("gather", l, w0, w1))
+        K1f, V1f = gathered[l]
+        K1f.record_stream(main); V1f.record_stream(main)
+        rk.phase_b(K1f, V1f)
+        b = ev(); b.record(main)
+        comm_stream.wait_event(b)
+        with torch.cuda.stream(comm_stream):
+            comm.reduce_scatter_heads(rk.gK1f, out=rk.gK1s)
+            comm.reduce_scatter_heads(rk.gV1f, out=rk.gV1s)
+            e = ev(); e.record(comm_stream)
+        r_done.append(e)
+    for l in range(len(layers) - 1, -1, -1):                   # Phase C, reverse layer order
+        w0 = ev(); w0.record(main)
+        main.wait_event(r_done[l])
+        w1 = ev(); w1.record(main)
+        waits.append(("reduce", l, w0, w1))
+        layers[l].phase_c(layers[l].gK1s, layers[l].gV1s)
+    return dict(waits=waits,
+                exposed_ms=lambda: {k: sum(a.elapsed_time(b) for kind, _, a, b in waits if kind == k)
+                                    for k in ("gather", "reduce")})

@@ -582,6 +582,34 @@ def test_split_group_schedule_on_one_gpu(ctx, world, wave):
     assert sorted(seen) == list(range(shape.N))               # every suffix ran on exactly one rank
 
 
+def test_split_group_multilayer_overlap_schedule(ctx):
+    """dist.run_split_group_layers: L layers with every layer's K1/V1 gather and gK1/gV1 reduction on a
+    communication stream, ordered against the compute stream by events only.  Run
+    with world = 1 (dist.SelfComm: the collectives are copies), so the result of every layer must
+    equal the unsharded oracle; the exposed waits are reported."""
+    from paper_2606_01143_b200 import dist as pfd
+    comm_stream = torch.cuda.Stream()
+    layers, refs = [], []
+    for l in range(3):
+        shape = inputs.small_case(4, 2, 128, 300, [129, 64, 200], seed=300 + l, dist="unit")
+        inp = inputs.make_group(shape)
+        refs.append(oracle.group_reference(inp))
+        layers.append(pfd.SplitGroupRank(ctx, inp, pfd.split_plan(shape, 1, 0), wave=2))
+    out = pfd.run_split_group_layers(layers, pfd.SelfComm(), comm_stream)
+    torch.cuda.synchronize()
+    exposed = out["exposed_ms"]()
+    assert set(exposed) == {"gather", "reduce"} and all(v >= 0.0 for v in exposed.values())
+    assert len(out["waits"]) == 6
+    for l, (rk, ref) in enumerate(zip(layers, refs)):
+        check(f"L{l} O1", rk.O1, ref.O1); check(f"L{l} dQ1", rk.dQ1, ref.dQ1)
+        check(f"L{l} dK1", rk.dK1, ref.dK1); check(f"L{l} dV1", rk.dV1, ref.dV1)
+        for pk in rk.pk:
+            for j, i in enumerate(pk["idx"]):
+                sl = slice(pk["cu"][j], pk["cu"][j + 1])
+                check(f"L{l} O2[{i}]", pk["O2"][sl], ref.O2[i]); check(f"L{l} dQ2[{i}]", pk["dQ2"][sl], ref.dQ2[i])
+                check(f"L{l} dK2[{i}]", pk["dK2"][sl], ref.dK2[i]); check(f"L{l} dV2[{i}]", pk["dV2"][sl], ref.dV2[i])
+
+
 @pytest.mark.parametrize("Hq,Hkv,d,segs", [
     (4, 2, 128, [130, 64, 200, 1, 127]),     # ragged segments, one of a single token
     (7, 1, 64, [64, 64, 64]),                # d = 64, GQA 7:1, exact tiles
