@@ -258,6 +258,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
             mbar_arrive(bar_Q);
         }
         float m_used = -INFINITY, l = 0.f;
+        int rng = 0, next_end = nP > 0 ? p.pre.tile0[1] - 1 : -1;   // last tile of the current prefix range
         for (int it = 0; it < n_iter; ++it) {
             const int b = it & 1;
             const uint32_t tS = tmem + b * 128 + qd * 32 + lane_off;     // this quarter of S[b]; P at its start
@@ -266,13 +267,16 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
             uint32_t x[32];
             tmem_ld32(tS, x);
             tmem_wait_ld();
-            // visible keys of this tile for this row, relative to this quarter's first column
-            int limit = t - (it - nP) * 128 + 1;
-            if (it < nP) {
-                int row0;
-                p.pre.locate(it, row0, limit);
+            // visible keys of this tile for this row, relative to this quarter's first column: only the
+            // last tile of a prefix range (ragged end) and the causal diagonal can hide any
+            int limit = 32;
+            if (it == n_iter - 1) {
+                limit = t - rb * 128 + 1 - qd * 32;
+            } else if (it == next_end) {
+                limit = p.pre.len[rng] - (it - p.pre.tile0[rng]) * 128 - qd * 32;
+                ++rng;
+                next_end = rng < p.pre.n ? p.pre.tile0[rng + 1] - 1 : -1;
             }
-            limit -= qd * 32;
             if (limit < 32) {                    // ragged prefix tail or causal diagonal
 #pragma unroll
                 for (int j = 0; j < 32; ++j)
