@@ -52,6 +52,11 @@ struct FwdParams {
     SeqTable seq;
 };
 
+template <int B>
+struct IntC {
+    static constexpr int v = B;
+};
+
 template <int D>
 struct FwdCfg {
     static constexpr int KS = 3;                       // K/V ring depth
@@ -259,8 +264,10 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
         }
         float m_used = -INFINITY, l = 0.f;
         int rng = 0, next_end = nP > 0 ? p.pre.tile0[1] - 1 : -1;   // last tile of the current prefix range
-        for (int it = 0; it < n_iter; ++it) {
-            const int b = it & 1;
+        // one KV tile; the S buffer index b = it & 1 is a compile-time constant (the loop below is
+        // unrolled by two): buffer addresses and barrier slots fold into immediates
+        auto tile_step = [&](auto bc, const int it) {
+            constexpr int b = decltype(bc)::v;
             const uint32_t tS = tmem + b * 128 + qd * 32 + lane_off;     // this quarter of S[b]; P at its start
             mbar_wait(&bar_S[b], (it >> 1) & 1);
             tc_fence_after();
@@ -336,6 +343,10 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
             tc_fence_before();
             mbar_arrive(&bar_P[2 * b + (qd >> 1)]);   // this half (64 keys) of P: two quarters arrive
             l += sum2.x + sum2.y;
+        };
+        for (int it = 0; it < n_iter; it += 2) {
+            tile_step(IntC<0>{}, it);
+            if (it + 1 < n_iter) tile_step(IntC<1>{}, it + 1);
         }
         // combine the four quarters' row sums, then each quarter normalises its quarter of the O columns
         float* xl = xch + (n_iter & 1) * 512;
