@@ -69,7 +69,7 @@ struct FwdCfg {
     static constexpr int OFF_X = OFF_BAR + 256;        // row-max / row-sum exchange between column halves
     static constexpr int SMEM = OFF_X + 2 * 4 * 128 * 4;
     static constexpr int THREADS = 576;
-    static constexpr int POLY16 = 5;                   // of 16 exp2 pairs, done by the polynomial on the FMA pipe
+    static constexpr int POLY16 = 6;                   // of 16 exp2 pairs, done by the polynomial on the FMA pipe
     static constexpr uint32_t T_O = 256, T_Q = 256 + D;  // TMEM columns of O and Q (S[b] at 128 b)
 };
 
