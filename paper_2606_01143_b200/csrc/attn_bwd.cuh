@@ -324,6 +324,7 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 // causal source: query t sees key kj iff t >= kj; only diagonal sub-tiles need it.
                 // prefix source: rows past the end of the tile's range (another node's keys) see nothing.
                 const bool diag = pre ? kvalid < 128 : iter.qs * 64 < kt * 128 + 128;
+                const float2 sc2 = make_float2(p.scale_log2, p.scale_log2);
                 const int col0 = iter.qs * 64 + w * 32 + 2 * lq;  // query (within its sequence) of r = 0, e = 0
 #pragma unroll
                 for (int blk = 0; blk < 2; ++blk) {
@@ -335,16 +336,19 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 #pragma unroll
                         for (int r = 0; r < 4; ++r) {
                             const int i = r * 4 + hf * 2;
-                            float p0 = fast_exp2(fmaf(__uint_as_float(s[blk][i]), p.scale_log2, -lv[r].x));
-                            float p1 = fast_exp2(fmaf(__uint_as_float(s[blk][i + 1]), p.scale_log2, -lv[r].y));
+                            // packed f32x2 arithmetic on the (query 2l, 2l+1) pair: one FFMA2 / FADD2 / FMUL2 each
+                            const float2 a = __ffma2_rn(make_float2(__uint_as_float(s[blk][i]), __uint_as_float(s[blk][i + 1])),
+                                                        sc2, make_float2(-lv[r].x, -lv[r].y));
+                            float2 pp = make_float2(fast_exp2(a.x), fast_exp2(a.y));
                             if (diag) {
-                                if (col0 + 8 * r < kj) p0 = 0.f;
-                                if (col0 + 8 * r + 1 < kj) p1 = 0.f;
+                                if (col0 + 8 * r < kj) pp.x = 0.f;
+                                if (col0 + 8 * r + 1 < kj) pp.y = 0.f;
                             }
-                            const float d0 = p0 * (__uint_as_float(dp[blk][i]) - dv[r].x);
-                            const float d1 = p1 * (__uint_as_float(dp[blk][i + 1]) - dv[r].y);
-                            pk[r * 2 + hf] = pack_bf16(p0, p1);
-                            const uint32_t dsv = pack_bf16(d0, d1);
+                            const float2 dd = __fmul2_rn(pp, __fadd2_rn(make_float2(__uint_as_float(dp[blk][i]),
+                                                                                    __uint_as_float(dp[blk][i + 1])),
+                                                                        make_float2(-dv[r].x, -dv[r].y)));
+                            pk[r * 2 + hf] = pack_bf16(pp.x, pp.y);
+                            const uint32_t dsv = pack_bf16(dd.x, dd.y);
                             dsk[r * 2 + hf] = dsv;
                             // dS^T -> smem, K-major swizzle-128B tile [128 keys][64 queries]
                             *reinterpret_cast<uint32_t*>(ds_tile + row * 128 + (((w * 4 + r) ^ (row & 7)) << 4) + lq * 4) = dsv;
