@@ -269,7 +269,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
         auto tile_step = [&](auto bc, const int it) {
             constexpr int b = decltype(bc)::v;
             const uint32_t tS = tmem + b * 128 + qd * 32 + lane_off;     // this quarter of S[b]; P at its start
-            mbar_wait(&bar_S[b], (it >> 1) & 1);
+            mbar_wait_short(&bar_S[b], (it >> 1) & 1);
             tc_fence_after();
             uint32_t x[32];
             tmem_ld32(tS, x);
