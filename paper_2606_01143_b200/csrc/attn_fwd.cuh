@@ -262,7 +262,8 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
             tc_fence_before();
             mbar_arrive(bar_Q);
         }
-        float m_used = -INFINITY, l = 0.f;
+        float m_used = -INFINITY, thr = -INFINITY;   // reference of the row and the rescale threshold m_used + 8
+        float2 l2 = make_float2(0.f, 0.f);           // row sum of this column quarter, as two partial sums
         int rng = 0, next_end = nP > 0 ? p.pre.tile0[1] - 1 : -1;   // last tile of the current prefix range
         // one KV tile; the S buffer index b = it & 1 is a compile-time constant (the loop below is
         // unrolled by two): buffer addresses and barrier slots fold into immediates
@@ -303,7 +304,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
             for (int o = 1; o < 4; ++o) mine = fmaxf(mine, xm[((qd + o) & 3) * 128 + r]);
             const float m_new = mine * c;
             // lazy rescale: keep a stale max while the new one is within 2^8 of it
-            const bool need = (it == 0) || (m_new > m_used + 8.f);
+            const bool need = (it == 0) || (m_new > thr);
             const unsigned rescale_mask = __ballot_sync(0xffffffffu, need && it > 0);
             if (rescale_mask != 0u) {
                 if ((tid & 31) == 0 && qd == 0)   // one of the row's four threads counts it
@@ -311,7 +312,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
                 mbar_wait(bar_PV, (it - 1) & 1); // P.V(it-1) must have landed in O
                 tc_fence_after();
                 const float alpha = need ? fast_exp2(m_used - m_new) : 1.f;
-                l *= alpha;
+                l2 = __fmul2_rn(l2, make_float2(alpha, alpha));
                 uint32_t o[DQ];
                 if constexpr (D == 128) tmem_ld32(tO, o); else tmem_ld16(tO, o);
                 tmem_wait_ld();
@@ -319,10 +320,9 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
                 for (int j = 0; j < DQ; ++j) o[j] = __float_as_uint(__uint_as_float(o[j]) * alpha);
                 if constexpr (D == 128) tmem_st32(tO, o); else tmem_st16(tO, o);
             }
-            if (need) m_used = m_new;
+            if (need) { m_used = m_new; thr = m_new + 8.f; }
             // ---- P = exp2(c S - m), packed to bf16 over the first 16 columns of this quarter of S
             const float2 c2 = make_float2(c, c), nm2 = make_float2(-m_used, -m_used);
-            float2 sum2 = make_float2(0.f, 0.f);
             uint32_t pk[16];
 #pragma unroll
             for (int j = 0; j < 16; ++j) {
@@ -335,14 +335,13 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
                     e.x = fast_exp2(a.x);
                     e.y = fast_exp2(a.y);
                 }
-                sum2 = __fadd2_rn(sum2, e);
+                l2 = __fadd2_rn(l2, e);
                 pk[j] = pack_bf16(e.x, e.y);
             }
             tmem_st16(tS, pk);
             tmem_wait_st();
             tc_fence_before();
             mbar_arrive(&bar_P[2 * b + (qd >> 1)]);   // this half (64 keys) of P: two quarters arrive
-            l += sum2.x + sum2.y;
         };
         for (int it = 0; it < n_iter; it += 2) {
             tile_step(IntC<0>{}, it);
@@ -350,6 +349,7 @@ attn_fwd_kernel(const __grid_constant__ CUtensorMap tmK1, const __grid_constant_
         }
         // combine the four quarters' row sums, then each quarter normalises its quarter of the O columns
         float* xl = xch + (n_iter & 1) * 512;
+        float l = l2.x + l2.y;
         xl[qd * 128 + r] = l;
         named_bar_sync(1 + (warp & 3), 128);
 #pragma unroll
