@@ -445,7 +445,8 @@ pf_status launch_fwd(pf_group* g, const pf_tensor& Q, const KvMaps* prefix, int6
 // ---- backward launch over a wave of n sequences packed along the token axis.  Keys of the prefix
 // source accumulate into accK1/accV1 (fp32, +=), keys of the causal source into accK2/accV2
 // (fp32 [total, Hkv, d], +=); dQ goes through the fp32 tile workspace and is rounded to bf16 once
-// all key tiles have contributed.
+// all key tiles have contributed.  zero_acc2: accK2/accV2 are scratch and are zero-filled here (by the
+// pre-processing launch) instead of accumulated onto.
 // `prefix` / `prefix_acc`: cached maps of the prefix source and of its accumulators (NULL when
 // Lp = 0); `causal` / `causal_acc`: cached maps when the causal source is the group's own K1/V1 and
 // gK1/gV1 (Phase C), else NULL and K2/V2/accK2/accV2 are encoded here.
@@ -454,7 +455,7 @@ pf_status launch_bwd(pf_group* g, const pf_tensor& Q, const KvMaps* prefix, cons
                      int64_t Lp, const KvMaps* causal, const KvMaps* causal_acc, const pf_tensor& K2,
                      const pf_tensor& V2, const pf_tensor& O, const float* LSE, int64_t lse_stride,
                      const pf_tensor& dO, float* accK2, float* accV2, const pf_tensor& dQ, int n,
-                     const int64_t* cu, int prof_kind, cudaStream_t s) {
+                     const int64_t* cu, int prof_kind, bool zero_acc2, cudaStream_t s) {
     pf_ctx* ctx = g->ctx;
     const int Hq = g->desc.n_q_heads, Hkv = g->desc.n_kv_heads, G = Hq / Hkv;
     const pf::SeqTable seq = make_seq_table(n, cu);
@@ -490,14 +491,15 @@ pf_status launch_bwd(pf_group* g, const pf_tensor& Q, const KvMaps* prefix, cons
     }
     const CUtensorMap &mK1 = prefix->k, &mV1 = prefix->v, &mK2 = causal->k, &mV2 = causal->v;
     const CUtensorMap &mAK1 = prefix_acc->k, &mAV1 = prefix_acc->v, &mAK2 = causal_acc->k, &mAV2 = causal_acc->v;
-    PF_CUDA(ctx, cudaMemsetAsync(dqacc, 0, size_t(npad) * Hq * D * 4, s));
-    {
+    {   // delta / lse2 and the zero fill of dqacc (npad * Hq * D floats) in one launch
         const int64_t threads = npad * (D / 8);
         dim3 grid(unsigned((threads + 255) / 256), Hq);
         pf::bwd_preprocess_kernel<D><<<grid, 256, 0, s>>>(
             static_cast<const __nv_bfloat16*>(O.ptr), O.stride_tok, O.stride_head,
             static_cast<const __nv_bfloat16*>(dO.ptr), dO.stride_tok, dO.stride_head, LSE, lse_stride,
-            lse2, delta, w.stat_stride, seq);
+            lse2, delta, w.stat_stride, reinterpret_cast<float4*>(dqacc),
+            reinterpret_cast<float4*>(zero_acc2 ? accK2 : nullptr), reinterpret_cast<float4*>(zero_acc2 ? accV2 : nullptr),
+            total * Hkv * (D / 4), seq);
         PF_CUDA(ctx, cudaGetLastError());
         ctx->n_launches += 1;
     }
@@ -935,18 +937,15 @@ pf_status pf_phaseB_bwd(pf_group* grp, int32_t n_seqs, const int32_t* cu_seqlens
         if (npad > grp->ws_cap)
             return fail(ctx, PF_WORKSPACE, "workspace too small for a suffix of %lld tokens", (long long)cu[1]);
         const int64_t tot = cu[n];
-        const size_t kvb = size_t(tot) * Hkv * d * 4;
-        PF_CUDA(ctx, cudaMemsetAsync(ak, 0, kvb, s));
-        PF_CUDA(ctx, cudaMemsetAsync(av, 0, kvb, s));
         const pf_tensor q = tok_offset(Q2, t0), k = tok_offset(K2, t0), v = tok_offset(V2, t0),
                         o = tok_offset(O2, t0), dout = tok_offset(dO2, t0), dq = tok_offset(dQ2, t0);
         if (d == 64) {
             st = launch_bwd<64>(grp, q, &grp->kv128, &grp->acc, grp->Lp, nullptr, nullptr, k, v, o,
-                                LSE2 + t0, total, dout, ak, av, dq, n, cu, 2, s);
+                                LSE2 + t0, total, dout, ak, av, dq, n, cu, 2, true, s);
             if (!st) st = launch_convert_kv2<64>(grp, ak, tok_offset(dK2, t0), av, tok_offset(dV2, t0), tot, s);
         } else {
             st = launch_bwd<128>(grp, q, &grp->kv128, &grp->acc, grp->Lp, nullptr, nullptr, k, v, o,
-                                 LSE2 + t0, total, dout, ak, av, dq, n, cu, 2, s);
+                                 LSE2 + t0, total, dout, ak, av, dq, n, cu, 2, true, s);
             if (!st) st = launch_convert_kv2<128>(grp, ak, tok_offset(dK2, t0), av, tok_offset(dV2, t0), tot, s);
         }
         if (st) return st;
@@ -1015,11 +1014,11 @@ pf_status pf_segment_bwd(pf_group* grp, int64_t Ls, pf_tensor Q, pf_tensor K, pf
     const int64_t cu[2] = {0, Ls};
     if (d == 64) {
         st = launch_bwd<64>(grp, Q, &grp->kv128, &grp->acc, grp->Lp, nullptr, nullptr, K, V, O, LSE, Ls,
-                            dO, accK, accV, dQ, 1, cu, 2, s);
+                            dO, accK, accV, dQ, 1, cu, 2, false, s);
         if (!st) st = launch_convert_kv2<64>(grp, accK, dK, accV, dV, Ls, s);
     } else {
         st = launch_bwd<128>(grp, Q, &grp->kv128, &grp->acc, grp->Lp, nullptr, nullptr, K, V, O, LSE, Ls,
-                             dO, accK, accV, dQ, 1, cu, 2, s);
+                             dO, accK, accV, dQ, 1, cu, 2, false, s);
         if (!st) st = launch_convert_kv2<128>(grp, accK, dK, accV, dV, Ls, s);
     }
     return st;
@@ -1050,19 +1049,16 @@ pf_status pf_phaseC_bwd(pf_group* grp, pf_tensor Q1, pf_tensor O1, const float* 
             if (align_up(Lp, 64) > grp->ws_cap) return fail(ctx, PF_WORKSPACE, "workspace too small");
             ak = reinterpret_cast<float*>(grp->ws + w.off_ak);
             av = reinterpret_cast<float*>(grp->ws + w.off_av);
-            const size_t kvb = size_t(Lp) * Hkv * d * 4;
-            PF_CUDA(ctx, cudaMemsetAsync(ak, 0, kvb, s));
-            PF_CUDA(ctx, cudaMemsetAsync(av, 0, kvb, s));
         }
         const int64_t cu[2] = {0, Lp};
         const KvMaps* cacc = grp->gK1 ? &grp->acc : nullptr;   // replay: workspace accumulators, encoded per call
         if (d == 64) {
             st = launch_bwd<64>(grp, Q1, nullptr, nullptr, 0, &grp->kv128, cacc, grp->K1, grp->V1, O1, LSE1,
-                                Lp, dO1, ak, av, dQ1, 1, cu, 3, s);
+                                Lp, dO1, ak, av, dQ1, 1, cu, 3, !grp->gK1, s);
             if (!st) st = launch_convert_kv2<64>(grp, ak, dK1, av, dV1, Lp, s);
         } else {
             st = launch_bwd<128>(grp, Q1, nullptr, nullptr, 0, &grp->kv128, cacc, grp->K1, grp->V1, O1, LSE1,
-                                 Lp, dO1, ak, av, dQ1, 1, cu, 3, s);
+                                 Lp, dO1, ak, av, dQ1, 1, cu, 3, !grp->gK1, s);
             if (!st) st = launch_convert_kv2<128>(grp, ak, dK1, av, dV1, Lp, s);
         }
         if (st) return st;
