@@ -63,18 +63,30 @@ rope_kernel(__nv_bfloat16* __restrict__ X, int64_t st, int64_t sh, int H, int d,
 // dW[M, N] (fp32, row-major) += X[L, M]^T dY[L, N]      (M = d_model, N = Hkv * d, K = tokens)
 // Both operands are read as they lie in memory -- token rows, feature columns contiguous -- i.e.
 // MN-major for the tensor core: A = X^T and B = dY come from TMA boxes of [64 tokens][64 features]
-// (swizzle-128B), no transpose pass.  CTA = one 128 x 128 tile of dW over a range of 64-token chunks
-// (grid.z splits the token range); fp32 accumulator = 128 TMEM columns; the epilogue adds the tile
-// into dW with vector reductions, so splits and successive calls (prefix term, suffix terms) sum.
+// (swizzle-128B), no transpose pass.  CTA = one (128 MH) x BN tile of dW over a range of 64-token
+// chunks (grid.z splits the token range); fp32 accumulators = MH x BN TMEM columns.  Tile size is what
+// bounds the main loop: a chunk of 64 tokens costs (128 MH + BN) x 128 bytes of L2 -> shared-memory
+// traffic for MH x BN / 2 clocks of MMA, i.e. 128 B/clk at 128 x 128, 64 B/clk at 256 x 256 against
+// the ~73 B/clk/SM the L2 delivers (profiles/r2_kernel_experiments.md).
+// Epilogue: each thread copies its accumulator row (BN fp32) from TMEM into the idle operand ring and
+// adds it into dW with ONE bulk reduce-add of BN x 4 contiguous bytes, so splits and successive calls
+// (prefix term, suffix terms) sum.
 //   warp 0 TMA producer | warp 1 TMEM alloc + tcgen05.mma issuer | warps 2-5 epilogue
 // ---------------------------------------------------------------------------------------------
+template <int MH, int BN>
 struct GemmCfg {
-    static constexpr int ST = 4;                       // ring depth
     static constexpr int SUB = 64 * 128;               // [64 tokens][64 bf16] box
-    static constexpr int STAGE = 4 * SUB;              // A: 2 boxes (128 features), B: 2 boxes
+    static constexpr int ABOX = 2 * MH, BBOX = BN / 64;
+    static constexpr int STAGE = (ABOX + BBOX) * SUB;
+    static constexpr int ST = (200 * 1024) / STAGE > 4 ? 4 : (200 * 1024) / STAGE;   // ring depth
     static constexpr int OFF_BAR = ST * STAGE;
     static constexpr int SMEM = OFF_BAR + 256;
     static constexpr int THREADS = 192;
+    static constexpr int TMEM_COLS = MH * BN;
+    static constexpr int EPI_ROW = BN * 4 + 16;        // staged accumulator row, padded against bank conflicts
+    static_assert(TMEM_COLS == 128 || TMEM_COLS == 256 || TMEM_COLS == 512, "TMEM allocation is a power of two");
+    static_assert(ST >= 3, "ring too shallow");
+    static_assert(128 * EPI_ROW <= OFF_BAR, "epilogue staging must fit the operand ring");
 };
 
 __device__ __forceinline__ void tma_load_2d(void* dst, const void* tmap, uint64_t* bar, int c0, int c1) {
@@ -84,17 +96,19 @@ __device__ __forceinline__ void tma_load_2d(void* dst, const void* tmap, uint64_
         ::"r"(smem_u32(dst)), "l"(reinterpret_cast<uint64_t>(tmap)), "r"(smem_u32(bar)), "r"(c0), "r"(c1)
         : "memory");
 }
-__device__ __forceinline__ void red_add_v4(float* dst, uint32_t a, uint32_t b, uint32_t c, uint32_t d) {
-    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};"
-                 ::"l"(dst), "f"(__uint_as_float(a)), "f"(__uint_as_float(b)), "f"(__uint_as_float(c)),
-                 "f"(__uint_as_float(d))
-                 : "memory");
+// shared -> global, element-wise fp32 add of `bytes` contiguous bytes (bulk async-group of the thread)
+__device__ __forceinline__ void bulk_red_add_row(float* dst, const void* src, uint32_t bytes) {
+    asm volatile(
+        "cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f32 [%0], [%1], %2;"
+        ::"l"(reinterpret_cast<uint64_t>(dst)), "r"(smem_u32(src)), "r"(bytes)
+        : "memory");
 }
 
+template <int MH, int BN>
 __global__ void __launch_bounds__(192, 1)
 kv_proj_grad_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmY,
                     float* __restrict__ dW, int n_cols, int n_chunks, int chunks_per_split) {
-    using C = GemmCfg;
+    using C = GemmCfg<MH, BN>;
     extern __shared__ __align__(1024) uint8_t smem[];
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::OFF_BAR);
     uint64_t* bar_full = bars;              // [ST]
@@ -103,7 +117,7 @@ kv_proj_grad_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_consta
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + 2 * C::ST + 1);
     const int tid = threadIdx.x, warp = tid >> 5;
     if ((smem_u32(smem) & 1023u) != 0) __trap();
-    const int m0 = blockIdx.x * 128, n0 = blockIdx.y * 128;
+    const int m0 = blockIdx.x * (128 * MH), n0 = blockIdx.y * BN;
     const int c_lo = blockIdx.z * chunks_per_split;
     const int n_it = min(n_chunks, c_lo + chunks_per_split) - c_lo;   // >= 1 by construction of the grid
 
@@ -112,7 +126,7 @@ kv_proj_grad_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_consta
         mbar_init(bar_done, 1);
         fence_mbar_init();
     }
-    if (warp == 1) tmem_alloc(tmem_slot, 128);
+    if (warp == 1) tmem_alloc(tmem_slot, C::TMEM_COLS);
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -126,49 +140,64 @@ kv_proj_grad_kernel(const __grid_constant__ CUtensorMap tmX, const __grid_consta
                 uint8_t* base = smem + st * C::STAGE;
                 mbar_wait(&bar_empty[st], ((it / C::ST) & 1) ^ 1);
                 mbar_arrive_expect_tx(&bar_full[st], C::STAGE);
-                tma_load_2d(base, &tmX, &bar_full[st], m0, k0);
-                tma_load_2d(base + C::SUB, &tmX, &bar_full[st], m0 + 64, k0);
-                tma_load_2d(base + 2 * C::SUB, &tmY, &bar_full[st], n0, k0);
-                tma_load_2d(base + 3 * C::SUB, &tmY, &bar_full[st], n0 + 64, k0);
+#pragma unroll
+                for (int i = 0; i < C::ABOX; ++i) tma_load_2d(base + i * C::SUB, &tmX, &bar_full[st], m0 + 64 * i, k0);
+#pragma unroll
+                for (int i = 0; i < C::BBOX; ++i)
+                    tma_load_2d(base + (C::ABOX + i) * C::SUB, &tmY, &bar_full[st], n0 + 64 * i, k0);
             }
         }
     } else if (warp == 1) {
         if (elect_one()) {
-            constexpr uint32_t idesc = make_idesc_bf16(128, 128, true, true);
+            constexpr uint32_t idesc = make_idesc_bf16(128, BN, true, true);
             for (int it = 0; it < n_it; ++it) {
                 const int st = it % C::ST;
                 const uint32_t sa = smem_u32(smem + st * C::STAGE);
-                const uint64_t ad = make_smem_desc_sw128(sa, C::SUB, 1024);                 // X^T, MN-major
-                const uint64_t bd = make_smem_desc_sw128(sa + 2 * C::SUB, C::SUB, 1024);    // dY, MN-major
+                const uint64_t ad = make_smem_desc_sw128(sa, C::SUB, 1024);                      // X^T, MN-major
+                const uint64_t bd = make_smem_desc_sw128(sa + C::ABOX * C::SUB, C::SUB, 1024);   // dY, MN-major
                 mbar_wait(&bar_full[st], (it / C::ST) & 1);
                 tc_fence_after();
 #pragma unroll
                 for (int kk = 0; kk < 4; ++kk)          // 16 tokens per instruction
-                    mma_ss(tmem, ad + ((kk * 2048) >> 4), bd + ((kk * 2048) >> 4), idesc, (it > 0 || kk > 0) ? 1u : 0u);
+#pragma unroll
+                    for (int mh = 0; mh < MH; ++mh)     // 128 features of X per instruction, dY shared
+                        mma_ss(tmem + mh * BN, ad + ((mh * 2 * C::SUB + kk * 2048) >> 4), bd + ((kk * 2048) >> 4),
+                               idesc, (it > 0 || kk > 0) ? 1u : 0u);
                 mma_commit(&bar_empty[st]);
             }
             mma_commit(bar_done);
         }
     } else {
-        // epilogue: thread <-> TMEM lane <-> row m of the tile; 128 fp32 columns added into dW
-        const int q = warp & 3;
+        // epilogue: thread <-> TMEM lane <-> row of a 128-row half.  bar_done = every MMA complete, hence
+        // every operand stage read: the ring is free and stages the rows.  A thread touches only its
+        // own staged row, so the only ordering needed is its own bulk group.
+        const int q = warp & 3, r = q * 32 + (tid & 31);
         const uint32_t lane_off = uint32_t(q * 32) << 16;
-        float* row = dW + int64_t(m0 + q * 32 + (tid & 31)) * n_cols + n0;
+        uint8_t* stage = smem + r * C::EPI_ROW;
         mbar_wait(bar_done, 0);
         tc_fence_after();
 #pragma unroll 1
-        for (int c = 0; c < 4; ++c) {
-            uint32_t v[32];
-            tmem_ld32(tmem + c * 32 + lane_off, v);
-            tmem_wait_ld();
+        for (int mh = 0; mh < MH; ++mh) {
+            if (mh > 0) bulk_wait_read<0>();            // the previous half's row has been read out
+#pragma unroll 1
+            for (int c = 0; c < BN / 32; ++c) {
+                uint32_t v[32];
+                tmem_ld32(tmem + mh * BN + c * 32 + lane_off, v);
+                tmem_wait_ld();
 #pragma unroll
-            for (int k = 0; k < 8; ++k)
-                red_add_v4(row + c * 32 + 4 * k, v[4 * k], v[4 * k + 1], v[4 * k + 2], v[4 * k + 3]);
+                for (int k = 0; k < 8; ++k)
+                    *reinterpret_cast<uint4*>(stage + c * 128 + k * 16) =
+                        make_uint4(v[4 * k], v[4 * k + 1], v[4 * k + 2], v[4 * k + 3]);
+            }
+            fence_proxy_async_smem();
+            bulk_red_add_row(dW + int64_t(m0 + mh * 128 + r) * n_cols + n0, stage, BN * 4);
+            bulk_commit();
         }
+        bulk_wait<0>();
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 1) tmem_dealloc(tmem, 128);
+    if (warp == 1) tmem_dealloc(tmem, C::TMEM_COLS);
 }
 
 

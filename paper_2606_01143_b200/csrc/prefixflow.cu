@@ -256,6 +256,18 @@ int64_t ws_capacity(const pf_desc& d, size_t bytes) {
     return (int64_t(bytes) - slack) / ws_bytes_per_pos(d) / 64 * 64;
 }
 
+template <int MH, int BN>
+bool set_gemm_attr() {
+    return cudaFuncSetAttribute(pf::kv_proj_grad_kernel<MH, BN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                pf::GemmCfg<MH, BN>::SMEM) == cudaSuccess;
+}
+template <int MH, int BN>
+void launch_gemm(dim3 grid, cudaStream_t s, const CUtensorMap& mX, const CUtensorMap& mY, float* dW, int n_cols,
+                 int n_chunks, int cps) {
+    pf::kv_proj_grad_kernel<MH, BN><<<grid, pf::GemmCfg<MH, BN>::THREADS, pf::GemmCfg<MH, BN>::SMEM, s>>>(
+        mX, mY, dW, n_cols, n_chunks, cps);
+}
+
 template <int D>
 pf_status set_attrs() {
     cudaError_t e;
@@ -632,9 +644,8 @@ pf_status pf_create(pf_ctx** out, int32_t device) {
         return PF_CUDA_ERROR;
     }
     ctx->encode = reinterpret_cast<EncodeTiledFn>(fn);
-    if (set_attrs<64>() != PF_OK || set_attrs<128>() != PF_OK ||
-        cudaFuncSetAttribute(pf::kv_proj_grad_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             pf::GemmCfg::SMEM) != cudaSuccess) {
+    if (set_attrs<64>() != PF_OK || set_attrs<128>() != PF_OK || !set_gemm_attr<1, 128>() ||
+        !set_gemm_attr<1, 256>() || !set_gemm_attr<2, 128>() || !set_gemm_attr<2, 256>()) {
         delete ctx;
         return PF_CUDA_ERROR;
     }
@@ -1142,15 +1153,21 @@ pf_status pf_kv_proj_grad(pf_ctx* ctx, int64_t L, int32_t d_model, int32_t n_col
         if (r != CUDA_SUCCESS)
             return fail(ctx, PF_CUDA_ERROR, "cuTensorMapEncodeTiled(%s) failed with CUresult %d", i ? "dY" : "X", int(r));
     }
-    const int tiles = (d_model / 128) * (n_cols / 128);
+    // the largest tile the shape divides into (256 x 256 halves the L2 -> shared-memory bytes per flop
+    // of 128 x 128); the token range is split so that one round of CTAs about fills the SMs
+    const int mh = d_model % 256 == 0 ? 2 : 1, bn = n_cols % 256 == 0 ? 256 : 128;
+    const int tiles = (d_model / (128 * mh)) * (n_cols / bn);
     const int n_chunks = int((L + 63) / 64);
-    int splits = (2 * ctx->num_sms + tiles - 1) / tiles;          // about two CTAs' worth of tiles per SM
+    int splits = ctx->num_sms / tiles;
     splits = splits < 1 ? 1 : (splits > n_chunks ? n_chunks : splits);
     const int cps = (n_chunks + splits - 1) / splits;
     splits = (n_chunks + cps - 1) / cps;                           // no empty split
-    dim3 grid(d_model / 128, n_cols / 128, splits);
-    pf::kv_proj_grad_kernel<<<grid, pf::GemmCfg::THREADS, pf::GemmCfg::SMEM, static_cast<cudaStream_t>(stream)>>>(
-        mX, mY, dW, n_cols, n_chunks, cps);
+    const dim3 grid(d_model / (128 * mh), n_cols / bn, splits);
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    if (mh == 2 && bn == 256) launch_gemm<2, 256>(grid, s, mX, mY, dW, n_cols, n_chunks, cps);
+    else if (mh == 2) launch_gemm<2, 128>(grid, s, mX, mY, dW, n_cols, n_chunks, cps);
+    else if (bn == 256) launch_gemm<1, 256>(grid, s, mX, mY, dW, n_cols, n_chunks, cps);
+    else launch_gemm<1, 128>(grid, s, mX, mY, dW, n_cols, n_chunks, cps);
     PF_CUDA(ctx, cudaGetLastError());
     ctx->n_launches += 1;
     return PF_OK;

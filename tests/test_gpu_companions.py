@@ -104,8 +104,11 @@ def test_rope_error_paths(ctx):
 @pytest.mark.parametrize("L,dm,Hkv,d", [
     (1, 128, 1, 128),
     (333, 256, 4, 128),        # ragged last 64-token chunk
-    (64, 128, 2, 64),
-    (5120, 3584, 4, 128),      # configs[1] prefix with a 7B-shaped d_model: 28 x 4 tiles, split over tokens
+    (64, 128, 2, 64),          # 128 x 128 tile
+    (200, 256, 1, 128),        # 256 x 128 tile
+    (200, 384, 2, 128),        # 128 x 256 tile
+    (5120, 3584, 4, 128),      # configs[1] prefix with a 7B-shaped d_model: 14 x 2 tiles of 256 x 256, split over tokens
+    (777, 512, 8, 128),        # 256 x 256 tiles, 2 x 4 of them, ragged token range split 13 ways
 ])
 def test_kv_proj_grad_matches_oracle(ctx, L, dm, Hkv, d):
     gen = torch.Generator().manual_seed(L + dm)
