@@ -672,3 +672,78 @@ def test_tree_structured_prefixes(ctx, Hq, Hkv, d, nodes):
     torch.cuda.synchronize()
     check("O", r["O"], ref["o"]); check("LSE", torch.cat(r["LSE"], 1), ref["lse"], lse=True)
     check("dQ", r["dQ"], ref["dq"]); check("dK", r["dK"], ref["dk"]); check("dV", r["dV"], ref["dv"])
+
+
+def _alloc_outputs_in_guarded_arena(g, guard=4096, fill=0xA5):
+    """schedule.alloc_outputs, but every output and the workspace is carved out of ONE byte arena with
+    `guard` bytes of a known pattern before and after it.  Returns (arena, owned-bytes mask)."""
+    dev = g.Q1.device
+    bf, f32 = torch.bfloat16, torch.float32
+    plan, off = [], guard
+
+    def want(key, shape, dt):
+        nonlocal off
+        nbytes = int(np.prod(shape)) * torch.empty((), dtype=dt).element_size()
+        plan.append((key, off, nbytes, tuple(shape), dt))
+        off += (nbytes + 255) // 256 * 256 + guard
+
+    d = g.d
+    want("O1", (g.Lp, g.Hq, d), bf); want("LSE1", (g.Hq, g.Lp), f32)
+    max_tok = 0
+    for w, pk in enumerate(g.packed):
+        tot = pk["cu"][-1]
+        max_tok = max(max_tok, tot)
+        for name, H in (("O2", g.Hq), ("dQ2", g.Hq), ("dK2", g.Hkv), ("dV2", g.Hkv)):
+            want((w, name), (tot, H, d), bf)
+        want((w, "LSE2"), (g.Hq, tot), f32)
+    for name, H, dt in (("gK1", g.Hkv, f32), ("gV1", g.Hkv, f32), ("dQ1", g.Hq, bf), ("dK1", g.Hkv, bf), ("dV1", g.Hkv, bf)):
+        want(name, (g.Lp, H, d), dt)
+    g.desc = pf.make_desc(g.Hq, g.Hkv, d)
+    want("workspace", (pf.pf_workspace_bytes(g.desc, g.Lp, max_tok),), torch.uint8)
+    arena = torch.full((off,), fill, dtype=torch.uint8, device=dev)
+    owned = torch.zeros((off,), dtype=torch.bool, device=dev)
+    for key, o, nbytes, shape, dt in plan:
+        assert o % 256 == 0
+        t = arena[o:o + nbytes].view(dt).view(shape)
+        owned[o:o + nbytes] = True
+        if isinstance(key, tuple):
+            g.packed[key[0]][key[1]] = t
+        else:
+            setattr(g, key, t)
+    g.O2, g.LSE2, g.dQ2, g.dK2, g.dV2 = [], [], [], [], []
+    for pk in g.packed:
+        cu = pk["cu"]
+        for j in range(len(pk["idx"])):
+            sl = slice(cu[j], cu[j + 1])
+            g.O2.append(pk["O2"][sl]); g.dQ2.append(pk["dQ2"][sl])
+            g.dK2.append(pk["dK2"][sl]); g.dV2.append(pk["dV2"][sl])
+            g.LSE2.append(pk["LSE2"][:, sl])
+    return arena, owned
+
+
+@pytest.mark.parametrize("Hq,Hkv,d,Lp,Ls,wave", [
+    (4, 2, 128, 333, [129, 1, 200, 77], 1),      # nothing a multiple of a tile
+    (4, 2, 128, 333, [129, 1, 200, 77], 3),      # packed waves of 3 + 1
+    (8, 2, 64, 130, [63, 65], 2),
+    (2, 1, 128, 0, [300], 1),                    # no prefix
+])
+def test_nothing_is_written_outside_the_outputs_and_inputs_stay_untouched(ctx, Hq, Hkv, d, Lp, Ls, wave):
+    """Bounds check of every kernel of the step (tile loads are clipped by the tensor maps, but the
+    helpers, the reduce-adds and the workspace layout index by hand): all outputs and the workspace
+    live in one arena between guard bands of a known byte pattern; after a step the bands are
+    intact, the read-only inputs are bit-identical, and the results still match the oracle."""
+    shape = inputs.small_case(Hq, Hkv, d, Lp, Ls, seed=77, dist="std")
+    inp = inputs.make_group(shape)
+    ref = oracle.group_reference(inp)
+    g = schedule.to_device(inp, wave=wave)
+    arena, owned = _alloc_outputs_in_guarded_arena(g)
+    before = [t.clone() for t in (g.Q1, g.K1, g.V1, g.dO1)] + \
+             [pk[n].clone() for pk in g.packed for n in ("Q2", "K2", "V2", "dO2")]
+    snaps = {}
+    schedule.run_prefixflow_step(ctx, g, after_each_suffix=lambda i: snaps.__setitem__(i, (g.gK1.clone(), g.gV1.clone())))
+    torch.cuda.synchronize()
+    assert bool((arena[~owned] == 0xA5).all()), "a kernel wrote outside its output / workspace"
+    after = [g.Q1, g.K1, g.V1, g.dO1] + [pk[n] for pk in g.packed for n in ("Q2", "K2", "V2", "dO2")]
+    for a, b in zip(before, after):
+        assert torch.equal(a.view(torch.int16), b.view(torch.int16)), "a read-only input was modified"
+    compare_group(g, ref, snaps, strict=True, backward=True, grad_rms_gate=STRICT_RMS_REL)
