@@ -175,3 +175,20 @@ def test_kv_proj_grad_error_paths(ctx):
     pf.pf_kv_proj_grad(ctx, X[:0], dY[:0], dW)                           # L = 0: no-op
     torch.cuda.synchronize()
     assert float(dW.abs().max()) == 0.0
+
+
+@pytest.mark.parametrize("L,dm,n_cols", [(130, 128, 128), (130, 256, 128), (130, 384, 256), (130, 256, 512)])
+def test_kv_proj_grad_writes_only_dW(ctx, L, dm, n_cols):
+    """dW sits between two guard bands of a known value: every tile variant's epilogue (one bulk
+    reduce-add per accumulator row) stays inside the [d_model, n_cols] matrix."""
+    gen = torch.Generator().manual_seed(11)
+    X, dY = _bf16(gen, L, dm).cuda(), _bf16(gen, L, n_cols).cuda()
+    guard = 1024
+    arena = torch.full((guard + dm * n_cols + guard,), 7.0, dtype=torch.float32, device="cuda")
+    dW = arena[guard:guard + dm * n_cols].view(dm, n_cols)
+    dW.zero_()
+    pf.pf_kv_proj_grad(ctx, X, dY, dW)
+    torch.cuda.synchronize()
+    assert bool((arena[:guard] == 7.0).all()) and bool((arena[guard + dm * n_cols:] == 7.0).all())
+    ref = oracle.kv_proj_grad(X.cpu().to(torch.float64).numpy(), dY.cpu().to(torch.float64).numpy(), [], [])
+    assert np.abs(dW.cpu().to(torch.float64).numpy() - ref).max() <= GEMM_MAX_REL * np.abs(ref).max() + GEMM_ABS
