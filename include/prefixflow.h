@@ -234,6 +234,32 @@ pf_status pf_offload(pf_ctx* ctx, const void* src_dev, void* dst_pinned_host, si
 pf_status pf_prefetch(pf_ctx* ctx, const void* src_pinned_host, void* dst_dev, size_t bytes,
                       void* side_stream);
 
+/* Allocation-free entry point, for callers that cannot call cudaMalloc (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid it): the backward of plain causal
+ * self-attention over ONE sequence of L tokens (the oracle's full-sequence causal pass,
+ * PAPER.md:194-198 with no prefix; the same kernels and the same result as pf_group_begin(Lp = L,
+ * K1 = K, V1 = V, no gK1/gV1, workspace) + pf_group_mark_cached + pf_phaseC_bwd), but with the
+ * workspace (softmax statistics, fp32 dQ^T tiles, fp32 dK/dV staging) in a scratch array built into
+ * the library: PF_STATIC_SCRATCH_BYTES = 32 MiB of device memory that every GPU loading the library
+ * holds until the process exits.  The call makes no cudaMalloc / cudaFree / event or stream
+ * creation and takes no caller workspace; inputs Q, O, dO [L, Hq, d], K, V [L, Hkv, d] bf16, LSE
+ * [Hq, L] fp32 (row stride L) and outputs dQ [L, Hq, d], dK, dV [L, Hkv, d] bf16 are the caller's
+ * device buffers as everywhere else.
+ *   Limit: align_up(L, 64) <= pf_causal_bwd_static_max_tokens(desc) (1792 tokens for 28/4 heads of
+ *   dim 128; 32 MiB / (8 Hq + 4 Hq d + 8 Hkv d) bytes per token); beyond it the call returns
+ *   PF_WORKSPACE with a message and enqueues nothing -- use pf_group_begin with your own workspace.
+ *   PF_STATE when the "profile" option is on (its bracket creates events).  L = 0 is a no-op.
+ *   The scratch keeps the previous call's contents; what must start at zero (dQ^T tiles, dK/dV
+ *   staging) is cleared by the call's own first kernel.  All calls, from every context and stream
+ *   of a device, share the one array: two calls that overlap on the GPU race; calls on one stream,
+ *   or ordered by events, are safe.  Its device address is taken once per context in pf_create. */
+#define PF_STATIC_SCRATCH_BYTES (32u << 20)
+size_t pf_static_scratch_bytes(void);
+int64_t pf_causal_bwd_static_max_tokens(const pf_desc* desc);
+pf_status pf_causal_bwd_static(pf_ctx* ctx, const pf_desc* desc, int64_t L, pf_tensor Q, pf_tensor K,
+                               pf_tensor V, pf_tensor O, const float* LSE, pf_tensor dO, pf_tensor dQ,
+                               pf_tensor dK, pf_tensor dV, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -25,7 +25,8 @@ SYMBOLS = ("pf_version", "pf_create", "pf_destroy", "pf_last_error", "pf_set_opt
            "pf_workspace_bytes", "pf_group_begin", "pf_phaseA_fwd", "pf_phaseB_fwd",
            "pf_phaseB_bwd", "pf_phaseC_bwd", "pf_group_end", "pf_offload", "pf_prefetch",
            "pf_counter", "pf_profile_read", "pf_group_mark_cached", "pf_segment_bwd",
-           "pf_group_set_prefix_ranges", "pf_rope", "pf_kv_proj_grad", "pf_bwd_split_model")
+           "pf_group_set_prefix_ranges", "pf_rope", "pf_kv_proj_grad", "pf_bwd_split_model",
+           "pf_static_scratch_bytes", "pf_causal_bwd_static_max_tokens", "pf_causal_bwd_static")
 
 
 class PrefixFlowError(RuntimeError):
@@ -101,6 +102,12 @@ def lib() -> ctypes.CDLL:
     L.pf_rope.argtypes = [vp, i32, pi32, i64, T, i32, i32, ctypes.c_float, i32, vp]
     L.pf_kv_proj_grad.restype = i32
     L.pf_kv_proj_grad.argtypes = [vp, i64, i32, i32, vp, i64, vp, i64, vp, vp]
+    L.pf_static_scratch_bytes.restype = ctypes.c_size_t
+    L.pf_static_scratch_bytes.argtypes = []
+    L.pf_causal_bwd_static_max_tokens.restype = i64
+    L.pf_causal_bwd_static_max_tokens.argtypes = [ctypes.POINTER(pf_desc)]
+    L.pf_causal_bwd_static.restype = i32
+    L.pf_causal_bwd_static.argtypes = [vp, ctypes.POINTER(pf_desc), i64, T, T, T, T, vp, T, T, T, T, vp]
     L.pf_offload.restype = i32
     L.pf_offload.argtypes = [vp, vp, vp, ctypes.c_size_t, vp]
     L.pf_prefetch.restype = i32
@@ -330,6 +337,23 @@ def pf_kv_proj_grad(ctx: _Handle, X: torch.Tensor, dY: torch.Tensor, dW: torch.T
         raise PrefixFlowError(PF_INVALID_ARG, f"pf_kv_proj_grad: dW must be a contiguous fp32 CUDA [{X.shape[1]}, {n_cols}] matrix")
     _check(lib().pf_kv_proj_grad(ctx.ptr, int(X.shape[0]), int(X.shape[1]), int(n_cols), _ptr(X), int(X.stride(0)),
                                  _ptr(dY), int(ldy), _ptr(dW), _stream(stream)), ctx)
+
+
+def pf_static_scratch_bytes() -> int:
+    return int(lib().pf_static_scratch_bytes())
+
+
+def pf_causal_bwd_static_max_tokens(desc: pf_desc) -> int:
+    return int(lib().pf_causal_bwd_static_max_tokens(ctypes.byref(desc)))
+
+
+def pf_causal_bwd_static(ctx: _Handle, desc: pf_desc, Q, K, V, O, LSE, dO, dQ, dK, dV, stream=None) -> None:
+    """Allocation-free causal backward of one sequence: the workspace is the library's built-in
+    32 MiB scratch (include/prefixflow.h); calls that overlap on the GPU race."""
+    L = int(Q.shape[0])
+    _check(lib().pf_causal_bwd_static(ctx.ptr, ctypes.byref(desc), L, as_tensor(Q), as_tensor(K), as_tensor(V),
+                                      as_tensor(O), _stat(LSE, Q.shape[1], L, "LSE"), as_tensor(dO),
+                                      as_tensor(dQ), as_tensor(dK), as_tensor(dV), _stream(stream)), ctx)
 
 
 def pf_offload(ctx: _Handle, src_dev: torch.Tensor, dst_pinned_host: torch.Tensor, stream) -> None:

@@ -31,7 +31,17 @@ constexpr int64_t kAlign = 256;
 constexpr size_t kMaxProfRecords = 1 << 16;   // unread profiling records kept per context
 inline int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
 
+// size of the built-in scratch of pf_causal_bwd_static (PF_STATIC_SCRATCH_BYTES in the header)
+constexpr size_t kStaticScratchBytes = size_t(32) << 20;
+
 }  // namespace
+
+// Built-in scratch of pf_causal_bwd_static: the backward's workspace (statistics, fp32 dQ^T tiles,
+// fp32 dK/dV staging) for callers that may not allocate.  Every GPU that loads the library holds
+// these 32 MiB until the process exits.  In host code this name is only a stand-in for the symbol:
+// the device address comes from cudaGetSymbolAddress (pf_create, once per context = per device, with
+// that device current) and is what the launches receive.
+static __device__ __align__(256) unsigned char pf_static_scratch[kStaticScratchBytes];
 
 struct ProfRec {
     cudaEvent_t a, b;
@@ -49,6 +59,7 @@ struct pf_ctx {
     int device = 0;
     int num_sms = 0;
     EncodeTiledFn encode = nullptr;
+    uint8_t* static_scratch = nullptr;   // device address of pf_static_scratch on this context's device
     int bwd_pairs_per_item = 0;  // (seq, head) pairs per prefix-tile CTA; 0 = heuristic
     int bwd_heads_per_item = 0;  // query heads per causal-tile CTA; 0 = heuristic
     bool profile = false;
@@ -649,6 +660,13 @@ pf_status pf_create(pf_ctx** out, int32_t device) {
         delete ctx;
         return PF_CUDA_ERROR;
     }
+    void* scratch = nullptr;   // the context's device is current here
+    e = cudaGetSymbolAddress(&scratch, pf_static_scratch);
+    if (e != cudaSuccess || !scratch) {
+        delete ctx;
+        return PF_CUDA_ERROR;
+    }
+    ctx->static_scratch = static_cast<uint8_t*>(scratch);
     *out = ctx;
     return PF_OK;
 }
@@ -1191,6 +1209,55 @@ pf_status pf_prefetch(pf_ctx* ctx, const void* src_pinned_host, void* dst_dev, s
     PF_CUDA(ctx, cudaMemcpyAsync(dst_dev, src_pinned_host, bytes, cudaMemcpyHostToDevice,
                                  static_cast<cudaStream_t>(side_stream)));
     return PF_OK;
+}
+
+size_t pf_static_scratch_bytes(void) { return kStaticScratchBytes; }
+
+int64_t pf_causal_bwd_static_max_tokens(const pf_desc* desc) {
+    if (!desc || desc->n_q_heads <= 0 || desc->n_kv_heads <= 0 || desc->head_dim <= 0) return 0;
+    return ws_capacity(*desc, kStaticScratchBytes);
+}
+
+pf_status pf_causal_bwd_static(pf_ctx* ctx, const pf_desc* desc, int64_t L, pf_tensor Q, pf_tensor K,
+                               pf_tensor V, pf_tensor O, const float* LSE, pf_tensor dO, pf_tensor dQ,
+                               pf_tensor dK, pf_tensor dV, void* stream) {
+    if (!ctx) return PF_INVALID_ARG;
+    pf_status st;
+    if ((st = check_device(ctx))) return st;
+    if ((st = check_desc(ctx, desc))) return st;
+    if (L < 0) return fail(ctx, PF_INVALID_ARG, "pf_causal_bwd_static: L < 0");
+    if (L == 0) return PF_OK;
+    if (ctx->profile)   // the profiling bracket creates events: not an allocation-free call
+        return fail(ctx, PF_STATE, "pf_causal_bwd_static: switch the \"profile\" option off (it creates CUDA events)");
+    if (!ctx->static_scratch) return fail(ctx, PF_STATE, "pf_causal_bwd_static: the built-in scratch has no device address");
+    const int64_t cap = ws_capacity(*desc, kStaticScratchBytes);
+    if (align_up(L, 64) > cap)
+        return fail(ctx, PF_WORKSPACE,
+                    "pf_causal_bwd_static: L=%lld exceeds the %lld tokens the built-in %zu-byte scratch holds for "
+                    "%d/%d heads of dim %d; use pf_group_begin with a workspace of your own",
+                    (long long)L, (long long)cap, kStaticScratchBytes, desc->n_q_heads, desc->n_kv_heads, desc->head_dim);
+    const int Hkv = desc->n_kv_heads, d = desc->head_dim;
+    if ((st = check_tensor(ctx, "K", K, L, Hkv, d))) return st;
+    if ((st = check_tensor(ctx, "V", V, L, Hkv, d))) return st;
+    // a group on the stack in the state pf_phaseC_bwd expects for the replay baseline (no gK1/gV1
+    // injection, dK/dV accumulated in the workspace): the workspace is the built-in scratch
+    pf_group g{};
+    g.ctx = ctx;
+    g.desc = *desc;
+    g.sigma = desc->softmax_scale > 0.f ? desc->softmax_scale : 1.0f / sqrtf(float(d));
+    g.Lp = L;
+    g.K1 = K;
+    g.V1 = V;
+    g.gK1 = nullptr;
+    g.gV1 = nullptr;
+    g.ws = ctx->static_scratch;
+    g.ws_bytes = kStaticScratchBytes;
+    g.ws_cap = cap;
+    g.pre = whole_prefix(L);
+    g.state = 1;
+    if ((st = make_map(ctx, &g.kv128.k, "K", K, L, Hkv, d, 128))) return st;
+    if ((st = make_map(ctx, &g.kv128.v, "V", V, L, Hkv, d, 128))) return st;
+    return pf_phaseC_bwd(&g, Q, O, LSE, dO, dQ, dK, dV, stream);
 }
 
 }  // extern "C"
