@@ -564,6 +564,19 @@ def main() -> None:
                      phaseB_tflops=tf(F["B_fwd"] + F["B_bwd"], bf_ms + bb_ms),
                      phaseB_pct_of_bf16_burst=100 * tf(F["B_fwd"] + F["B_bwd"], bf_ms + bb_ms) / peaks["burst"],
                      speedup_vs_replay=(replay["ms_per_step"] / ms1) if replay else None)
+        # the same with the Phase-B forwards on a second stream (schedule.run_prefixflow_step(fwd_stream=...)):
+        # the forward of suffix i+1 runs beside the backward of suffix i and fills the SMs that the
+        # last round of CTAs of either launch leaves idle (224 forward CTAs on 148 SMs per suffix)
+        side = torch.cuda.Stream(dev)
+        step1s = lambda: schedule.run_prefixflow_step(ctx, g1, stream, fwd_stream=side)
+        for _ in range(args.warmup):
+            step1s()
+        ms1s = timed(step1s, args.steps)
+        wave1["fwd_side_stream"] = dict(ms_per_step=ms1s, tflops=world * F["step"] / (ms1s * 1e-3) / 1e12,
+                                        speedup_vs_one_stream=ms1 / ms1s,
+                                        speedup_vs_replay=(replay["ms_per_step"] / ms1s) if replay else None,
+                                        note="Phase-B forwards enqueued on a second stream; every backward waits for its own forward")
+        del step1s
         # the rejected gK/gV organisation, measured next to the shipped one: every
         # suffix adds into a partial accumulator of its own, one reduce pass before Phase C
         pK = torch.empty((shape.N, shape.Lp, shape.n_kv_heads, shape.head_dim), dtype=torch.float32, device=dev)
@@ -596,7 +609,12 @@ def main() -> None:
             ms_g1 = timed(gr1.replay, args.steps)
             graph["wave1_ms_per_step"] = ms_g1
             graph["wave1_speedup_vs_eager"] = wave1["ms_per_step"] / ms_g1
-            del gr1, g1
+            del gr1
+            gr1s = schedule.capture_step(ctx, g1, fwd_stream=torch.cuda.Stream(dev))   # fork / join captured
+            for _ in range(2):
+                gr1s.replay()
+            graph["wave1_fwd_side_stream_ms_per_step"] = timed(gr1s.replay, args.steps)
+            del gr1s, g1
         torch.cuda.empty_cache()
 
     # ---- companions: RoPE of one wave's Q2 and K2 (HBM-bound) and the

@@ -100,16 +100,33 @@ def alloc_outputs(g: DeviceGroup) -> None:
 
 
 def run_prefixflow_step(ctx, g: DeviceGroup, stream=None, after_each_suffix=None,
-                        order: Optional[Sequence[int]] = None) -> None:
+                        order: Optional[Sequence[int]] = None, fwd_stream=None) -> None:
     """Phase A -> Phase B (fwd, bwd) per suffix wave -> Phase C.
-    `order` permutes the waves (= the suffixes when wave == 1)."""
+    `order` permutes the waves (= the suffixes when wave == 1).
+
+    `fwd_stream` (a torch.cuda.Stream other than `stream`): the Phase-B forwards are enqueued there
+    instead.  They read only Q2/K2/V2 and the cached K1/V1 (inputs of the step), so the
+    forward of wave i+1 may run while the backward of wave i does, and the first one beside Phase A:
+    the SMs a launch leaves idle in its last round of CTAs are picked up by the other stream's launch.
+    Every backward waits for its own forward; the forwards of a step wait for everything enqueued on
+    `stream` before it (the previous step's backward still reads O2 / LSE2)."""
+    main = stream if isinstance(stream, torch.cuda.Stream) else None
+    if fwd_stream is not None:
+        if main is None:
+            if stream is not None:
+                raise ValueError("fwd_stream needs `stream` as a torch.cuda.Stream (or None = the current stream)")
+            main = torch.cuda.current_stream()
+        fwd_stream.wait_stream(main)
     grp = pf.pf_group_begin(ctx, g.desc, g.Lp, g.K1, g.V1, g.gK1, g.gV1, g.workspace, stream)
     try:
         pf.pf_phaseA_fwd(grp, g.Q1, g.O1, g.LSE1, stream)
         for i in (range(len(g.packed)) if order is None else order):
             pk = g.packed[i]
             cu = pk["cu"]
-            pf.pf_phaseB_fwd(grp, cu, pk["Q2"], pk["K2"], pk["V2"], pk["O2"], pk["LSE2"], stream)
+            pf.pf_phaseB_fwd(grp, cu, pk["Q2"], pk["K2"], pk["V2"], pk["O2"], pk["LSE2"],
+                             stream if fwd_stream is None else fwd_stream)
+            if fwd_stream is not None:
+                main.wait_stream(fwd_stream)   # (an event recorded on fwd_stream here; later forwards are not waited for)
             pf.pf_phaseB_bwd(grp, cu, pk["Q2"], pk["K2"], pk["V2"], pk["O2"], pk["LSE2"], pk["dO2"],
                              pk["dQ2"], pk["dK2"], pk["dV2"], stream)
             if after_each_suffix is not None:
@@ -155,20 +172,22 @@ class _nullctx:
         return False
 
 
-def capture_step(ctx, g: DeviceGroup, order: Optional[Sequence[int]] = None) -> "torch.cuda.CUDAGraph":
+def capture_step(ctx, g: DeviceGroup, order: Optional[Sequence[int]] = None,
+                 fwd_stream=None) -> "torch.cuda.CUDAGraph":
     """One A -> B -> C step captured into a CUDA graph.  Every C-ABI call only enqueues memsets and
     kernels on the caller's stream (tensor maps and kernel parameters are baked in at capture), so a
     training loop whose buffers keep their addresses replays the whole step with one launch; the
     launch gaps between the ~18 (one packed wave) to ~60 (one call per suffix) dependent kernels of
-    a step go away.  The profile option must be off during capture."""
+    a step go away.  The profile option must be off during capture.  With `fwd_stream` the fork to and
+    the joins from the forwards' stream are captured too (every forward is joined by its backward)."""
     side = torch.cuda.Stream(g.Q1.device)
     side.wait_stream(torch.cuda.current_stream(g.Q1.device))
     with torch.cuda.stream(side):                 # warm-up outside the capture (lazy module loads)
-        run_prefixflow_step(ctx, g, side, order=order)
+        run_prefixflow_step(ctx, g, side, order=order, fwd_stream=fwd_stream)
     torch.cuda.current_stream(g.Q1.device).wait_stream(side)
     graph = torch.cuda.CUDAGraph()
     with torch.cuda.graph(graph, stream=side):
-        run_prefixflow_step(ctx, g, torch.cuda.current_stream(g.Q1.device), order=order)
+        run_prefixflow_step(ctx, g, torch.cuda.current_stream(g.Q1.device), order=order, fwd_stream=fwd_stream)
     return graph
 
 

@@ -263,6 +263,32 @@ def test_cuda_graph_replay_matches_oracle(ctx, wave):
         compare_group(g, ref)
 
 
+@pytest.mark.parametrize("wave", [1, 2, 0])
+def test_forwards_on_a_side_stream_match_oracle(ctx, wave):
+    """schedule.run_prefixflow_step(fwd_stream=...): the Phase-B forwards run on a second stream beside
+    Phase A and the previous wave's backward (they depend on inputs only).  Three steps
+    back to back on the same buffers (the next step's forwards must wait for this step's backwards,
+    which still read O2 / LSE2), then every output and the per-suffix gK1/gV1 snapshots against the oracle."""
+    shape = inputs.small_case(8, 2, 128, 700, [129, 64, 300, 1, 200], seed=53, dist="std")
+    inp = inputs.make_group(shape)
+    ref = oracle.group_reference(inp)
+    g = schedule.to_device(inp, wave=wave if wave else shape.N)
+    side = torch.cuda.Stream()
+    snaps = {}
+    for rep in range(3):
+        schedule.run_prefixflow_step(ctx, g, fwd_stream=side,
+                                     after_each_suffix=lambda i: snaps.__setitem__(i, (g.gK1.clone(), g.gV1.clone())))
+    torch.cuda.synchronize()
+    compare_group(g, ref, snaps, strict=True, backward=True, grad_rms_gate=STRICT_RMS_REL)
+    # and from a CUDA graph: the fork / join of the two streams is captured with the step
+    for t in (g.O1, g.dQ1, g.dK1, g.dV1, *(pk[n] for pk in g.packed for n in ("O2", "dQ2", "dK2", "dV2"))):
+        t.zero_()
+    gr = schedule.capture_step(ctx, g, fwd_stream=side)
+    gr.replay(); gr.replay()
+    torch.cuda.synchronize()
+    compare_group(g, ref, None, strict=True, backward=True, grad_rms_gate=STRICT_RMS_REL)
+
+
 def _random_shapes(count, seed):
     rng = np.random.default_rng(seed)
     out = []
