@@ -252,7 +252,7 @@ pf_status pf_prefetch(pf_ctx* ctx, const void* src_pinned_host, void* dst_dev, s
  *   The scratch keeps the previous call's contents; what must start at zero (dQ^T tiles, dK/dV
  *   staging) is cleared by the call's own first kernel.  All calls, from every context and stream
  *   of a device, share the one array: two calls that overlap on the GPU race; calls on one stream,
- *   or ordered by events, are safe.  Its device address is taken once per context in pf_create. */
+ *   or ordered by events, are safe.  Its device address is taken once per device in pf_create. */
 #define PF_STATIC_SCRATCH_BYTES (32u << 20)
 size_t pf_static_scratch_bytes(void);
 int64_t pf_causal_bwd_static_max_tokens(const pf_desc* desc);

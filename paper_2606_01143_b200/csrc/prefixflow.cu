@@ -10,6 +10,7 @@
 #include <cmath>
 #include <algorithm>
 #include <functional>
+#include <mutex>
 #include <new>
 #include <queue>
 #include <vector>
@@ -33,6 +34,7 @@ inline int64_t align_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
 
 // size of the built-in scratch of pf_causal_bwd_static (PF_STATIC_SCRATCH_BYTES in the header)
 constexpr size_t kStaticScratchBytes = size_t(32) << 20;
+constexpr int kMaxDevices = 64;
 
 }  // namespace
 
@@ -660,13 +662,22 @@ pf_status pf_create(pf_ctx** out, int32_t device) {
         delete ctx;
         return PF_CUDA_ERROR;
     }
-    void* scratch = nullptr;   // the context's device is current here
-    e = cudaGetSymbolAddress(&scratch, pf_static_scratch);
-    if (e != cudaSuccess || !scratch) {
-        delete ctx;
-        return PF_CUDA_ERROR;
+    {   // device address of the built-in scratch: looked up once per device (this context's device is
+        // current here), remembered for later contexts on the same device
+        static std::mutex mu;
+        static void* addr[kMaxDevices] = {nullptr};
+        std::lock_guard<std::mutex> lock(mu);
+        void* scratch = device >= 0 && device < kMaxDevices ? addr[device] : nullptr;
+        if (!scratch) {
+            e = cudaGetSymbolAddress(&scratch, pf_static_scratch);
+            if (e != cudaSuccess || !scratch) {
+                delete ctx;
+                return PF_CUDA_ERROR;
+            }
+            if (device >= 0 && device < kMaxDevices) addr[device] = scratch;
+        }
+        ctx->static_scratch = static_cast<uint8_t*>(scratch);
     }
-    ctx->static_scratch = static_cast<uint8_t*>(scratch);
     *out = ctx;
     return PF_OK;
 }
