@@ -35,6 +35,17 @@ def test_version_and_workspace_bytes_are_host_only():
     assert pf.pf_workspace_bytes(d, -1, 0) == 0
 
 
+def test_static_scratch_limits_are_host_only():
+    """pf_causal_bwd_static's limit is computable without a GPU: 32 MiB / bytes per token, a multiple of 64."""
+    assert pf.pf_static_scratch_bytes() == 32 << 20
+    d = pf.make_desc(28, 4, 128)
+    cap = pf.pf_causal_bwd_static_max_tokens(d)
+    per_tok = 8 * 28 + 4 * 28 * 128 + 8 * 4 * 128
+    assert cap % 64 == 0 and cap == ((32 << 20) - 6 * 256) // per_tok // 64 * 64 == 1792
+    assert pf.pf_causal_bwd_static_max_tokens(pf.make_desc(2, 2, 64)) > cap
+    assert pf.pf_workspace_bytes(d, cap, 0) > 32 << 20 >= cap * per_tok   # the caller-side formula keeps 16 x 64 spare rows
+
+
 def test_struct_layout_matches_header():
     assert ctypes.sizeof(pf.pf_desc) == 16
     assert ctypes.sizeof(pf.pf_tensor) == 24
