@@ -45,6 +45,8 @@ struct BwdParams {
     int chunksP, ppcP;             // prefix items: the n*G (seq, head) pairs in chunks of ppcP
     int chunksC, ppcC;             // causal items: the G heads of the sequence in chunks of ppcC
     int nItemsP;                   // nPT * Hkv * chunksP
+    int interleave;                // 1: each chunk's prefix items are followed by the causal items of the
+                                   //    sequences whose last pair the chunk holds (else: all prefix items first)
     float scale_log2;              // sigma * log2(e)
     float sigma;
     SeqTable seq;
@@ -146,6 +148,21 @@ attn_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 
     // ---- item decode: prefix-source items first (heaviest), then the causal key tiles ----
     int item = blockIdx.x;
+    if (p.interleave && p.nItemsP > 0) {
+        // launch order chunk by chunk: prefix items of chunk c, then the causal items of the sequences
+        // that chunk c completes, while their Q / dO and dQ^T tiles are still in L2.  Translated here
+        // into the item numbering of the plain order (prefix items first), which the decode below uses.
+        const int perP = p.nPT * p.Hkv, perC = p.Hkv * p.chunksC, pairs = p.seq.n * p.G;
+        int base = 0, s_lo = 0;
+        for (int c = 0; c < p.chunksP; ++c) {
+            const int s_hi = min(pairs, (c + 1) * p.ppcP) / p.G;     // sequences complete after chunk c
+            const int nC = (p.seq.ckt[s_hi] - p.seq.ckt[s_lo]) * perC;
+            if (item < base + perP) { item = c * perP + (item - base); break; }
+            if (item < base + perP + nC) { item = p.nItemsP + p.seq.ckt[s_lo] * perC + (item - base - perP); break; }
+            base += perP + nC;
+            s_lo = s_hi;
+        }
+    }
     const bool pre = item < p.nItemsP;
     int kt, g, pair_lo, pair_hi, qs_lo, kvrow0, kvalid = 128;   // kvalid: rows of the tile inside its prefix range
     if (pre) {

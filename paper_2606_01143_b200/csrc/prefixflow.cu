@@ -52,7 +52,7 @@ struct ProfRec {
 
 // key / value of the backward item-split model (choose_split below)
 struct SplitEntry {
-    int n, nPT, Hkv, G;
+    int n, nPT, Hkv, G, interleave;
     int cu[pf::kMaxSeqs + 1];
     int ppcP, ppcC;
 };
@@ -64,6 +64,7 @@ struct pf_ctx {
     uint8_t* static_scratch = nullptr;   // device address of pf_static_scratch on this context's device
     int bwd_pairs_per_item = 0;  // (seq, head) pairs per prefix-tile CTA; 0 = heuristic
     int bwd_heads_per_item = 0;  // query heads per causal-tile CTA; 0 = heuristic
+    int bwd_interleave = 1;      // 1 (default): causal items launched right behind the prefix chunk that completes their sequence
     bool profile = false;
     bool zero_accumulators = true;
     bool deterministic_gkv = false;  // one CTA per key tile: gK1/gV1/dK/dV sums in a fixed order
@@ -379,6 +380,39 @@ struct SplitModel {
         }
         return *std::max_element(h.begin(), h.end());
     }
+    // the interleaved launch order: chunk by chunk, prefix items then the causal items of the sequences
+    // the chunk completes
+    double interleaved(int ppcP, int ppcC, std::vector<double>& h) const {
+        h.assign(sms, 0.0);
+        const int pairs = n * G;
+        int s_lo = 0;
+        for (int lo = 0; lo < pairs; lo += ppcP) {
+            const int hi = std::min(pairs, lo + ppcP);
+            double it = 0;
+            for (int pr = lo; pr < hi; ++pr) it += seq.pqs[pr / G + 1] - seq.pqs[pr / G];
+            int64_t cnt = int64_t(nPT) * Hkv;
+            const double cost = it + kC0;
+            if (cnt >= sms && *std::max_element(h.begin(), h.end()) - h[0] <= cost) {
+                const double add = cost * double(cnt / sms);
+                for (double& v : h) v += add;
+                cnt %= sms;
+            }
+            for (; cnt > 0; --cnt) give(h, cost);
+            const int s_hi = hi / G;
+            for (int s = s_lo; s < s_hi; ++s) {
+                const int nqs = seq.pqs[s + 1] - seq.pqs[s], nkt = seq.ckt[s + 1] - seq.ckt[s];
+                for (int kt = 0; kt < nkt; ++kt) {
+                    const int rows = std::max(0, nqs - 2 * kt);
+                    for (int g = 0; g < Hkv; ++g)
+                        for (int c0 = 0; c0 < G; c0 += ppcC)
+                            give(h, rows > 0 ? double(std::min(G, c0 + ppcC) - c0) * rows + kC0 : 0.5);
+                }
+            }
+            s_lo = s_hi;
+        }
+        return *std::max_element(h.begin(), h.end());
+    }
+    bool interleave = false;
     void choose(int& ppcP, int& ppcC) const {
         const int pairs = n * G;
         static const int kChunks[] = {1, 2, 3, 4, 5, 6, 7, 8, 10, 12, 14, 16, 20, 24, 28, 32, 40, 48, 56, 64, 96, 128};
@@ -399,10 +433,15 @@ struct SplitModel {
         double bm = 1e300;
         std::vector<double> after_prefix, h;
         for (int a : as) {
-            prefix_phase(a, after_prefix);
+            if (!(interleave && nPT > 0)) prefix_phase(a, after_prefix);
             for (int b : bs) {
-                h = after_prefix;
-                const double m = causal_phase(b, h);
+                double m;
+                if (interleave && nPT > 0) {
+                    m = interleaved(a, b, h);
+                } else {
+                    h = after_prefix;
+                    m = causal_phase(b, h);
+                }
                 if (getenv("PF_SPLIT_DEBUG")) fprintf(stderr, "split a=%d b=%d makespan=%.1f\n", a, b, m);
                 // ties (0.2 %): fewer, longer items -- less K/V re-loading, and CTAs that run side by
                 // side then walk the same query heads, which keeps their Q / dO tiles in L2 (measured at
@@ -544,14 +583,16 @@ pf_status launch_bwd(pf_group* g, const pf_tensor& Q, const KvMaps* prefix, cons
     } else {
         SplitEntry key;
         memset(&key, 0, sizeof(key));
-        key.n = n; key.nPT = p.nPT; key.Hkv = Hkv; key.G = G;
+        key.n = n; key.nPT = p.nPT; key.Hkv = Hkv; key.G = G; key.interleave = ctx->bwd_interleave;
         for (int i = 0; i <= n; ++i) key.cu[i] = seq.cu[i];
         const SplitEntry* hit = nullptr;
         for (const SplitEntry& e : ctx->split_cache)
             if (memcmp(&e, &key, offsetof(SplitEntry, ppcP)) == 0) { hit = &e; break; }
         if (!hit) {
             key.ppcP = ppcP; key.ppcC = ppcC;
-            SplitModel{seq, n, p.nPT, Hkv, G, ctx->num_sms}.choose(key.ppcP, key.ppcC);
+            SplitModel model{seq, n, p.nPT, Hkv, G, ctx->num_sms};
+            model.interleave = ctx->bwd_interleave != 0;
+            model.choose(key.ppcP, key.ppcC);
             if (ctx->split_cache.size() >= 64) ctx->split_cache.erase(ctx->split_cache.begin());
             ctx->split_cache.push_back(key);
             hit = &ctx->split_cache.back();
@@ -566,6 +607,7 @@ pf_status launch_bwd(pf_group* g, const pf_tensor& Q, const KvMaps* prefix, cons
     p.ppcP = ppcP; p.chunksP = (pairs + ppcP - 1) / ppcP;
     p.ppcC = ppcC; p.chunksC = (G + ppcC - 1) / ppcC;
     p.nItemsP = p.nPT * Hkv * p.chunksP;
+    p.interleave = ctx->bwd_interleave && !ctx->deterministic_gkv;
     p.scale_log2 = g->sigma * 1.4426950408889634f;
     p.sigma = g->sigma;
     const int64_t items = int64_t(p.nItemsP) + int64_t(seq.ckt[n]) * Hkv * p.chunksC;
@@ -697,6 +739,10 @@ const char* pf_last_error(const pf_ctx* ctx) { return ctx ? ctx->err : "pf_ctx i
 
 pf_status pf_set_option(pf_ctx* ctx, const char* name, int64_t value) {
     if (!ctx || !name) return PF_INVALID_ARG;
+    if (strcmp(name, "bwd_interleave") == 0) {
+        ctx->bwd_interleave = value != 0;
+        return PF_OK;
+    }
     if (strcmp(name, "bwd_pairs_per_item") == 0 || strcmp(name, "bwd_heads_per_item") == 0) {
         if (value < 0 || value > (1 << 20)) return fail(ctx, PF_INVALID_ARG, "%s must be >= 0", name);
         (name[4] == 'p' ? ctx->bwd_pairs_per_item : ctx->bwd_heads_per_item) = int(value);
@@ -744,7 +790,9 @@ pf_status pf_bwd_split_model(const pf_desc* desc, int64_t Lp, int32_t n_seqs, co
     const pf::SeqTable seq = make_seq_table(n_seqs, cu);
     const int G = desc->n_q_heads / desc->n_kv_heads;
     int a = n_seqs * G > 0 ? n_seqs * G : 1, b = (G + 1) / 2;
-    SplitModel{seq, n_seqs, int((Lp + 127) / 128), desc->n_kv_heads, G, n_sms}.choose(a, b);
+    SplitModel model{seq, n_seqs, int((Lp + 127) / 128), desc->n_kv_heads, G, n_sms};
+    model.interleave = true;   // the default launch order ("bwd_interleave" = 1)
+    model.choose(a, b);
     *pairs_per_item = a;
     *heads_per_item = b;
     return PF_OK;

@@ -747,6 +747,25 @@ def _alloc_outputs_in_guarded_arena(g, guard=4096, fill=0xA5):
     return arena, owned
 
 
+@pytest.mark.parametrize("interleave", [0, 1])
+@pytest.mark.parametrize("items", [None, (1, 1), (3, 2), (5, 1), (1000, 1000)])
+@pytest.mark.parametrize("Hq,Hkv,d,Lp,Ls,wave", [
+    (8, 2, 128, 700, [129, 64, 300, 1, 200], 0),      # pairs per item that cut sequences in the middle
+    (6, 2, 128, 333, [200] * 7, 3),                   # packed waves of 3 + 3 + 1
+    (4, 4, 128, 130, [63, 65], 2),                    # G = 1
+])
+def test_bwd_launch_orders(ctx, interleave, items, Hq, Hkv, d, Lp, Ls, wave):
+    """Option "bwd_interleave": the causal-tile items right behind the prefix chunk that completes their
+    sequence (default) or all prefix-tile items first -- the same items, the same sums, for every item
+    split including chunks that end in the middle of a sequence's heads."""
+    shape = inputs.small_case(Hq, Hkv, d, Lp, Ls, seed=11, dist="std")
+    pf.pf_set_option(ctx, "bwd_interleave", interleave)
+    try:
+        run_and_compare(ctx, shape, items=items, wave=wave if wave else shape.N)
+    finally:
+        pf.pf_set_option(ctx, "bwd_interleave", 1)
+
+
 @pytest.mark.parametrize("Hq,Hkv,d,Lp,Ls,wave", [
     (4, 2, 128, 333, [129, 1, 200, 77], 1),      # nothing a multiple of a tile
     (4, 2, 128, 333, [129, 1, 200, 77], 3),      # packed waves of 3 + 1

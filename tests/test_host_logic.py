@@ -43,13 +43,14 @@ def test_wave_partition_and_ragged_recipe():
 def test_bwd_split_model_is_host_only_deterministic_and_even():
     """The backward item split comes from a list-scheduling simulation on the host (prefixflow.cu
     SplitModel): no GPU needed.  configs[1], one packed wave on 148 SMs: 8 x 7 = 56 pairs in 4 even
-    chunks of 14 -- the split measured fastest on the B200 (profiles/r2_kernel_experiments.md)."""
+    chunks of 14 with all prefix items first, 5 chunks of 12 in the default interleaved launch order
+    (profiles/r2_kernel_experiments.md)."""
     from paper_2606_01143_b200 import binding as pf
     d = pf.make_desc(28, 4, 128)
     cu8 = [1024 * i for i in range(9)]
     a, b = pf.pf_bwd_split_model(d, 5120, cu8)
     assert (a, b) == pf.pf_bwd_split_model(d, 5120, cu8)
-    assert a == 14 and 56 % a == 0 and 1 <= b <= 7
+    assert 8 <= a <= 14 and 1 <= b <= 7          # 4-7 chunks of the 56 pairs: about one round of CTAs per chunk
     # Phase C / replay: no prefix source, one sequence: only the heads-per-item choice matters
     a1, b1 = pf.pf_bwd_split_model(d, 0, [0, 5120])
     assert 1 <= b1 <= 7 and a1 >= 1
